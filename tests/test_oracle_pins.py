@@ -1,0 +1,316 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU, no CUDA path).
+
+Each test names the passage it checks (PAPER.md = /root/reference/PAPER.md; pins P1..P9 of
+SURVEY.md 8(c)).  A plausible mistake in oracle/rt_oracle.cpp -- a dropped term, an increment
+with the wrong propensity, a wrong draw index, a missing tie rule, a firing past t_end -- fails
+at least one of them.
+"""
+import ctypes
+import math
+import os
+import subprocess
+from fractions import Fraction
+
+import numpy as np
+import pytest
+from scipy import stats
+
+import oracle
+import rt_workloads as W
+from helpers.direct_method import direct_method
+from helpers.exact_kurtz import exact_path
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+INF = math.inf
+
+
+# ------------------------------------------------------------------ P1: Philox4x32-10
+def _kat_rows():
+    rows = []
+    with open(os.path.join(HERE, "golden", "philox4x32_10_kat.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            v = [int(x, 16) for x in line.split()]
+            rows.append((v[0:4], v[4:6], v[6:10]))
+    return rows
+
+
+def test_philox_known_answers():
+    """Random123 known-answer vectors (Salmon et al. SC'11)."""
+    rows = _kat_rows()
+    assert len(rows) == 3
+    for ctr, key, out in rows:
+        assert list(oracle.philox4x32_10(ctr, key)) == out
+
+
+def test_philox_matches_cuda_toolkit_header(tmp_path):
+    """Same function as the CUDA toolkit's curand_Philox4x32_10 (host-compiled header)."""
+    inc = "/usr/local/cuda/include"
+    if not os.path.exists(os.path.join(inc, "curand_philox4x32_x.h")):
+        pytest.skip("CUDA toolkit header not present")
+    so = str(tmp_path / "libtk_philox.so")
+    subprocess.run(["g++", "-O1", "-shared", "-fPIC", "-I", inc, "-o", so,
+                    os.path.join(HERE, "helpers", "curand_philox_host.cpp")], check=True)
+    tk = ctypes.CDLL(so)
+    rng = np.random.default_rng(123)
+    for _ in range(2000):
+        ctr = rng.integers(0, 2**32, size=4, dtype=np.uint64).astype(np.uint32)
+        key = rng.integers(0, 2**32, size=2, dtype=np.uint64).astype(np.uint32)
+        out = np.zeros(4, dtype=np.uint32)
+        tk.toolkit_philox4x32_10(ctr.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)),
+                                 key.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)),
+                                 out.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)))
+        assert list(oracle.philox4x32_10(ctr, key)) == list(out)
+
+
+def test_exp_draw_is_unit_exponential_and_keyed():
+    """Eq.23: Delta T = ln(1/r).  Draws are unit exponentials, strictly finite
+    (reading G5: r in (0,1]), and every key component (seed, trajectory, k, n) matters."""
+    e = np.array([oracle.exp_draw(11, 3, k, n) for k in range(200) for n in range(100)])
+    assert np.all(np.isfinite(e)) and np.all(e >= 0.0)
+    assert stats.kstest(e, "expon").pvalue > 0.01
+    assert abs(e.mean() - 1.0) < 3.0 / math.sqrt(e.size)
+    base = oracle.exp_draw(5, 6, 7, 8)
+    assert base == oracle.exp_draw(5, 6, 7, 8)
+    variants = [oracle.exp_draw(4, 6, 7, 8), oracle.exp_draw(5, 5, 7, 8),
+                oracle.exp_draw(5, 6, 6, 8), oracle.exp_draw(5, 6, 7, 9),
+                oracle.exp_draw(5 + (1 << 32), 6, 7, 8), oracle.exp_draw(5, 6 + (1 << 32), 7, 8),
+                oracle.exp_draw(5, 6, 8, 7), oracle.exp_draw(6, 5, 7, 8)]
+    assert len(set(variants + [base])) == len(variants) + 1
+    # the mapping itself: U = (u53+1) 2^-53 from words w0 (low) and w1 (high) of the block
+    w = oracle.philox4x32_10([7, 8, 6, 0], [5, 0])
+    u53 = ((int(w[1]) << 32) | int(w[0])) >> 11
+    assert base == pytest.approx(-math.log((u53 + 1) / 2.0**53), rel=4e-16)
+
+
+# ------------------------------------------------------------------ P8: combinatorial factor
+def test_binomial_factor_matches_math_comb():
+    """Eq.2, reading G1/G2: h = prod_j C(X_j, sigma_jk), exact integers."""
+    for sigma in (1, 2, 3):
+        for x in list(range(0, 60)) + [1000, 65535, 2**21 - 1]:
+            assert oracle.binom(x, sigma) == math.comb(x, sigma)
+    assert oracle.binom(2**31 - 1, 2) == math.comb(2**31 - 1, 2)
+
+
+def test_propensity_is_rate_times_product_of_binomials():
+    """Eq.1-2 against exact rational arithmetic."""
+    net, x0, _ = W.make_config("cfg3", scale=0.01)
+    a = oracle.propensities(net, x0)
+    rp, rs, rg = net["react_ptr"], net["react_species"], net["react_sigma"]
+    for k in range(net["n_reactions"]):
+        exact = Fraction(float(net["rate"][k]))
+        for e in range(rp[k], rp[k + 1]):
+            exact *= math.comb(int(x0[rs[e]]), int(rg[e]))
+        assert a[k] == pytest.approx(float(exact), rel=4e-16)
+    assert (a[np.diff(rp) == 0] == net["rate"][np.diff(rp) == 0]).all()
+
+
+def test_dimerisation_needs_two_molecules():
+    """2A -> B: C(1,2) = 0 so X0=1 is absorbed at once; X0=2 fires exactly once, at a time
+    ~ Exp(c * C(2,2))."""
+    c = 0.7
+    net = W.from_reactions(2, [({0: 2}, {1: 1}, c)])
+    r = oracle.run(net, [1, 0], seed=3, max_firings=10)
+    assert (r["firings"], r["stop"], r["t"]) == (0, oracle.STOP_ABSORBED, 0.0)
+    assert list(r["x"]) == [1, 0]
+    times = []
+    for traj in range(4000):
+        r = oracle.run(net, [2, 0], seed=3, trajectory=traj, max_firings=10, trace_cap=4)
+        assert r["firings"] == 1 and r["stop"] == oracle.STOP_ABSORBED
+        assert list(r["x"]) == [0, 1]
+        times.append(r["trace_t"][0])
+    assert stats.kstest(np.array(times) * c, "expon").pvalue > 0.01
+
+
+def test_pure_death_is_binomial():
+    """X -> 0 with rate c from n molecules: X(t) ~ Binomial(n, exp(-c t))."""
+    c, n0, t_end, n_traj = 0.5, 40, 1.3, 4000
+    net = W.from_reactions(1, [({0: 1}, {}, c)])
+    out = oracle.ensemble(net, [n0], seed=21, traj_first=0, n_traj=n_traj, t_end=t_end)
+    assert np.all(out["stop"] == oracle.STOP_T_END) and np.all(out["t"] == t_end)
+    x = out["x"][:, 0]
+    p = math.exp(-c * t_end)
+    assert abs(x.mean() - n0 * p) < 3 * math.sqrt(n0 * p * (1 - p) / n_traj)
+    obs = np.bincount(x, minlength=n0 + 1).astype(float)
+    exp = stats.binom.pmf(np.arange(n0 + 1), n0, p) * n_traj
+    keep = exp >= 5
+    chi2 = ((obs[keep] - exp[keep]) ** 2 / exp[keep]).sum() + \
+        (obs[~keep].sum() - exp[~keep].sum()) ** 2 / max(exp[~keep].sum(), 1e-9)
+    assert stats.chi2.sf(chi2, keep.sum()) > 0.001
+
+
+# ------------------------------------------------------------------ P2: one constant channel
+def test_single_source_channel_closed_form():
+    """0 -> X with constant a = c: internal time runs at rate c, so the n-th firing happens at
+    t_n = (E_0 + ... + E_{n-1}) / c  (Eq.15, Eq.23-24).  Pins the draw index (k, n), the
+    trajectory/seed keying, the (T,P) bookkeeping and the loop order."""
+    c, seed, traj, n = 3.7, 99, 12345678901, 500
+    net = W.from_reactions(1, [({}, {0: 1}, c)])
+    r = oracle.run(net, [0], seed=seed, trajectory=traj, max_firings=n, trace_cap=n)
+    assert r["firings"] == n and r["stop"] == oracle.STOP_MAX_FIRINGS
+    assert list(r["trace_mu"]) == [0] * n and r["x"][0] == n
+    e = [oracle.exp_draw(seed, traj, 0, i) for i in range(n + 1)]
+    for i in (0, 1, 2, 17, n - 1):
+        assert r["trace_t"][i] == pytest.approx(math.fsum(e[:i + 1]) / c, rel=1e-13)
+    assert r["P"][0] == pytest.approx(math.fsum(e), rel=1e-13)       # next target: n+1 draws
+    assert r["T"][0] == pytest.approx(math.fsum(e[:n]), rel=1e-13)   # internal time at t_n
+    assert r["fire_count"][0] == n
+
+
+# ------------------------------------------------------------------ exact path (Eq.15-16)
+@pytest.mark.parametrize("case", ["lv", "dimer", "mixed"])
+def test_matches_exact_rational_path(case):
+    """The oracle's firing sequence and times equal the exact (rational arithmetic) sample path
+    of the random time-change representation Eq.16 driven by the same unit-Poisson jump times:
+    checks that T_k advances with the propensity that held DURING each interval, that only the
+    fired channel's target moves (Eq.26) and that X += v_mu (Eq.5)."""
+    if case == "lv":
+        net, x0 = W.lotka_volterra(y1=40, y2=30, c2=0.05)
+    elif case == "dimer":
+        net = W.from_reactions(2, [({0: 2}, {1: 1}, 0.02), ({1: 1}, {0: 2}, 0.9)])
+        x0 = [30, 5]
+    else:
+        net = W.from_reactions(3, [({}, {0: 1}, 4.0), ({0: 1, 1: 2}, {2: 1}, 0.01),
+                                   ({2: 1}, {1: 2}, 0.5), ({0: 3}, {1: 1}, 0.002),
+                                   ({1: 1}, {}, 0.1)])
+        x0 = [12, 9, 3]
+    seed, traj, n = 17, 5, 300
+    r = oracle.run(net, x0, seed=seed, trajectory=traj, max_firings=n, trace_cap=n)
+    path, xf = exact_path(net, x0, lambda k, i: oracle.exp_draw(seed, traj, k, i), n)
+    assert r["firings"] == len(path) == n
+    assert list(r["trace_mu"]) == [mu for mu, _ in path]
+    for got, (_, want) in zip(r["trace_t"], path):
+        assert got == pytest.approx(float(want), rel=1e-11)
+    assert list(r["x"]) == xf
+
+
+def test_tie_goes_to_lowest_index():
+    """Reading G6: equal waiting times -> lowest k.  Two channels whose clamped residual is 0
+    (reading G7) tie at Delta t = 0; +inf ties (all a_k = 0) mean ABSORBED."""
+    net = W.from_reactions(1, [({0: 1}, {}, 1.0), ({0: 1}, {}, 2.0)])
+    r = oracle.run(net, [0], seed=1, max_firings=5)
+    assert (r["firings"], r["stop"]) == (0, oracle.STOP_ABSORBED)
+
+
+# ------------------------------------------------------------------ P3/P4: birth-death
+def test_birth_death_stationary_poisson():
+    """Config 1: 0->X (c1=10), X->0 (c2=0.1), X0=0, t_end=1000, Philox seed 1:
+    X(t_end) ~ Poisson(c1/c2 = 100) (north_star).  Also P4: births R_0 ~ Poisson(c1 t_end) and
+    T_0(t_end) = c1 t_end (Eq.10, Eq.15), and t == t_end exactly (reading G8)."""
+    net, x0, p = W.make_config("cfg1")
+    n_traj = p["n_traj"]
+    out = oracle.ensemble(net, x0, seed=p["seed"], traj_first=0, n_traj=n_traj,
+                          max_firings=p["max_firings"], t_end=p["t_end"], n_threads=4)
+    assert np.all(out["stop"] == oracle.STOP_T_END) and np.all(out["t"] == p["t_end"])
+    x = out["x"][:, 0].astype(float)
+    assert abs(x.mean() - 100.0) < 3 * math.sqrt(100.0 / n_traj)
+    assert abs(x.var(ddof=1) - 100.0) < 3 * 100.0 * math.sqrt(2.0 / (n_traj - 1))
+    # discrete law: compare the empirical CDF with Poisson(100) (KS statistic, conservative)
+    d = np.abs(np.searchsorted(np.sort(x), np.arange(40, 170), side="right") / n_traj
+               - stats.poisson.cdf(np.arange(40, 170), 100.0)).max()
+    assert d < 1.63 / math.sqrt(n_traj)          # 1% point of the Kolmogorov distribution
+    births = (out["firings"].astype(float) + x) / 2.0    # firings = births + deaths, x = births - deaths
+    assert abs(births.mean() - 1e4) < 3 * math.sqrt(1e4 / n_traj)
+    r = oracle.run(net, x0, seed=1, trajectory=0, max_firings=p["max_firings"], t_end=p["t_end"])
+    assert r["T"][0] == pytest.approx(10.0 * 1000.0, rel=1e-12)
+    assert r["fire_count"][0] - r["fire_count"][1] == r["x"][0]
+
+
+def test_birth_death_transient_at_fixed_time():
+    """X(t) ~ Poisson((c1/c2)(1 - exp(-c2 t))) from X0 = 0 at a short fixed time: a loop that
+    fired once past t_end (the paper's `while t < t_max`, reading G8) would bias this."""
+    net, x0, _ = W.make_config("cfg1")
+    t_end, n_traj = 5.0, 6000
+    lam = 100.0 * (1.0 - math.exp(-0.1 * t_end))
+    out = oracle.ensemble(net, x0, seed=8, traj_first=100, n_traj=n_traj, t_end=t_end, n_threads=4)
+    x = out["x"][:, 0].astype(float)
+    assert abs(x.mean() - lam) < 3 * math.sqrt(lam / n_traj)
+    assert abs(x.var(ddof=1) - lam) < 3 * lam * math.sqrt(2.0 / (n_traj - 1))
+
+
+# ------------------------------------------------------------------ P5/P6: identities
+@pytest.mark.parametrize("name,scale,firings", [("cfg3", 0.02, 3000), ("cfg4", 0.002, 3000),
+                                                ("cfg2", 1.0, 5000)])
+def test_kurtz_identity_and_invariants(name, scale, firings):
+    """Eq.5: X = X0 + sum_k R_k v_k exactly; counts stay >= 0; t and the trace
+    are non-decreasing; sum R_k = firings; 0 <= T_k <= P_k (to rounding) with T_k = 0 and
+    P_k = E(k,0) for channels that never had a_k > 0 ... (Eq.15, Eq.26)."""
+    net, x0, p = W.make_config(name, scale=scale)
+    M = net["n_reactions"]
+    r = oracle.run(net, x0, seed=p["seed"], max_firings=firings, trace_cap=firings)
+    assert r["firings"] == firings
+    x = np.array(x0, dtype=np.int64)
+    sp, ss, sv = net["stoich_ptr"], net["stoich_species"], net["stoich_v"]
+    for k in np.flatnonzero(r["fire_count"]):
+        x[ss[sp[k]:sp[k + 1]]] += int(r["fire_count"][k]) * sv[sp[k]:sp[k + 1]]
+    assert (x == r["x"]).all() and (r["x"] >= 0).all()
+    assert int(r["fire_count"].sum()) == firings
+    assert (np.bincount(r["trace_mu"], minlength=M) == r["fire_count"]).all()
+    assert (np.diff(r["trace_t"]) >= 0).all() and r["t"] == r["trace_t"][-1]
+    assert (r["T"] >= 0).all() and (r["T"] <= r["P"] * (1 + 1e-12)).all()
+    # P_k is the sum of the first n_k + 1 draws of channel k
+    for k in list(np.argsort(-r["fire_count"].astype(np.int64))[:5]) + [0, M - 1]:
+        want = math.fsum(oracle.exp_draw(p["seed"], 0, int(k), i)
+                         for i in range(int(r["fire_count"][k]) + 1))
+        assert r["P"][k] == pytest.approx(want, rel=1e-13)
+    # a shorter run is a prefix of a longer one (determinism contract)
+    r2 = oracle.run(net, x0, seed=p["seed"], max_firings=firings // 3, trace_cap=firings)
+    assert (r2["trace_mu"] == r["trace_mu"][:firings // 3]).all()
+    assert (r2["trace_t"] == r["trace_t"][:firings // 3]).all()
+
+
+def test_t_end_stop_advances_internal_time_only():
+    """Reading G8: at t_end nothing fires, t = t_end, T_k += a_k (t_end - t)."""
+    net, x0 = W.lotka_volterra()
+    full = oracle.run(net, x0, seed=2, max_firings=200, trace_cap=200)
+    t_cut = 0.5 * (full["trace_t"][99] + full["trace_t"][100])
+    cut = oracle.run(net, x0, seed=2, t_end=t_cut, trace_cap=200)
+    assert cut["stop"] == oracle.STOP_T_END and cut["t"] == t_cut and cut["firings"] == 100
+    assert (cut["trace_mu"] == full["trace_mu"][:100]).all()
+    ref = oracle.run(net, x0, seed=2, max_firings=100)
+    a = oracle.propensities(net, ref["x"])
+    assert (cut["x"] == ref["x"]).all() and (cut["P"] == ref["P"]).all()
+    np.testing.assert_allclose(cut["T"], ref["T"] + a * (t_cut - ref["t"]), rtol=1e-14)
+
+
+# ------------------------------------------------------------------ P7: race of exponentials
+def test_race_of_exponentials():
+    """Eq.21 and Eq.25: with constant propensities a_k the first
+    firing is channel k with probability a_k / sum a, at a time ~ Exp(sum a)."""
+    c = np.array([0.5, 2.0, 1.0, 4.5])
+    net = W.from_reactions(4, [({}, {k: 1}, float(c[k])) for k in range(4)])
+    n_traj = 8000
+    mus, ts = [], []
+    for traj in range(n_traj):
+        r = oracle.run(net, [0] * 4, seed=31, trajectory=traj, max_firings=1, trace_cap=1)
+        mus.append(r["trace_mu"][0])
+        ts.append(r["trace_t"][0])
+    obs = np.bincount(mus, minlength=4)
+    assert stats.chisquare(obs, c / c.sum() * n_traj).pvalue > 0.001
+    assert stats.kstest(np.array(ts) * c.sum(), "expon").pvalue > 0.01
+
+
+# ------------------------------------------------------------------ P9: brute-force SSA
+def _two_sample(xa, xb):
+    assert stats.ks_2samp(xa, xb).pvalue > 0.01
+    se = math.sqrt(xa.var(ddof=1) / xa.size + xb.var(ddof=1) / xb.size)
+    assert abs(xa.mean() - xb.mean()) < 3 * se + 1e-12
+
+
+@pytest.mark.parametrize("case", ["birth_death", "dimer", "lv"])
+def test_agrees_in_distribution_with_direct_method(case):
+    """The random-time algorithm is an exact SSA: marginals at t_end agree with an
+    independent Gillespie direct method (own RNG, own propensity code)."""
+    if case == "birth_death":
+        (net, x0), t_end, n_traj = W.birth_death(), 30.0, 2000
+    elif case == "dimer":
+        net = W.from_reactions(2, [({0: 2}, {1: 1}, 0.01), ({1: 1}, {0: 2}, 1.0)])
+        x0, t_end, n_traj = [100, 0], 2.0, 2000
+    else:
+        (net, x0), t_end, n_traj = W.lotka_volterra(), 0.3, 1500
+    out = oracle.ensemble(net, x0, seed=77, traj_first=0, n_traj=n_traj, t_end=t_end, n_threads=4)
+    assert np.all(out["stop"] == oracle.STOP_T_END)
+    xd, _ = direct_method(net, x0, n_traj, t_end, seed=1234)
+    for j in range(net["n_species"]):
+        _two_sample(out["x"][:, j].astype(float), xd[:, j].astype(float))
