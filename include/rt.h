@@ -1,0 +1,158 @@
+/* rt.h -- C ABI of the B200-native random-time (NRRTA) stochastic simulation hot path.
+ *
+ * Method: Liu & Wang, "Parallel implementations of random time algorithm for chemical network
+ * stochastic simulations", arXiv 2103.00405 (PAPER.md = the extracted text).  One firing is:
+ *   a_k   = c_k * prod_j C(X_j, sigma_jk)                 Eq.1-2
+ *   dt_k  = (P_k - T_k) / a_k   (+inf if a_k = 0)         Eq.24, a_k constant
+ *   mu    = argmin_k dt_k, ties to the lowest k           Eq.25
+ *   t    += dt_mu;  T_k += a_k * dt_mu for EVERY k        Eq.15
+ *   X    += v_mu                                          Eq.5
+ *   P_mu += -ln U, U from Philox4x32-10 keyed by          Eq.23,26
+ *           (seed, trajectory, reaction, firing count)
+ * Loop shape: Table 1 / Table 3; both a time and a step limit as in the
+ * paper's model file.  All arithmetic is IEEE binary64, every operation
+ * rounded to nearest separately (no fused multiply-add); DESIGN.md lists the readings taken
+ * where the paper is silent or garbled.
+ *
+ * Conventions.  Every function returns an int: RT_OK (0) or a negative RT_ERR_* code; nothing
+ * throws across the boundary.  Pointers are HOST pointers unless the name ends in _dev or the
+ * parameter is documented as a device pointer.  The caller owns every array passed in and every
+ * output buffer; the library copies what it needs during the call and keeps no caller pointer.
+ * Results depend only on (network, x0, seed, trajectory, limits) -- not on the launch shape,
+ * on how an ensemble is batched, nor on the propensity refresh mode.
+ */
+#ifndef RT_B200_H_
+#define RT_B200_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- status codes ------------------------------------------------------------------------ */
+#define RT_OK                0
+#define RT_ERR_NULL         -1   /* a required pointer is NULL                                   */
+#define RT_ERR_BAD_NETWORK  -2   /* rt_network fails validation (see rt_validate_network)        */
+#define RT_ERR_BAD_ARG      -3   /* x0 < 0 or above the count bound, t_end NaN or < 0, no limit  */
+#define RT_ERR_UNSUPPORTED  -4   /* sigma > 3, or more than 2^32-1 CSR entries                   */
+#define RT_ERR_OVERFLOW     -5   /* a species count left [0, bound] during a run                 */
+#define RT_ERR_CUDA         -6   /* CUDA runtime error, no device, or an in-kernel barrier timeout */
+#define RT_ERR_OOM          -7   /* host or device allocation failed                             */
+
+/* ---- why a trajectory stopped (not errors) ------------------------------------------------- */
+#define RT_STOP_T_END        1   /* next firing would pass t_end: t = t_end, nothing fired        */
+#define RT_STOP_MAX_FIRINGS  2   /* max_firings reactions fired                                  */
+#define RT_STOP_ABSORBED     3   /* every propensity is 0; t stays at the last firing             */
+
+typedef struct rt_model rt_model;   /* opaque; owns the device copy of the network and all state */
+
+/* Reaction network in CSR form (N >= 1 species, M >= 1 reactions, reactant
+ * coefficients sigma_jk, net change v_k; sparse matrices).  Row k of the react_*
+ * arrays lists the reactant species of reaction k with sigma_jk >= 1; row k of the stoich_*
+ * arrays lists the species whose count changes when k fires, with v_jk != 0.  A species may
+ * appear at most once per row, and v_jk >= -sigma_jk' must hold (a reaction cannot remove more
+ * than it requires, so counts stay >= 0).  rate[k] = c_k, finite and >= 0. */
+typedef struct {
+  int32_t n_species;               /* N >= 1 */
+  int32_t n_reactions;             /* M >= 1 */
+  const int64_t *react_ptr;        /* [M+1], react_ptr[0] = 0, non-decreasing                    */
+  const int32_t *react_species;    /* [react_ptr[M]] species index in [0, N)                     */
+  const int32_t *react_sigma;      /* [react_ptr[M]] 1 <= sigma <= 3                             */
+  const int64_t *stoich_ptr;       /* [M+1]                                                      */
+  const int32_t *stoich_species;   /* [stoich_ptr[M]]                                            */
+  const int32_t *stoich_v;         /* [stoich_ptr[M]] v != 0                                     */
+  const double  *rate;             /* [M]                                                        */
+} rt_network;
+
+/* Per-trajectory outcome.  24 bytes, no padding surprises: (f64, u64, i32, i32). */
+typedef struct {
+  double   t;         /* simulated time reached                                                   */
+  uint64_t firings;   /* reactions fired                                                          */
+  int32_t  stop;      /* RT_STOP_*                                                                */
+  int32_t  status;    /* RT_OK or RT_ERR_OVERFLOW for this trajectory                             */
+} rt_result;
+
+/* Count bound: species counts must stay in [0, 2^31-1] when every sigma <= 2 and in
+ * [0, 2^21-1] when some sigma = 3, so that C(X, sigma) is exact in int64 (G2). */
+
+/* Host-only check of a network (no GPU needed).  RT_OK, RT_ERR_NULL, RT_ERR_BAD_NETWORK
+ * (N < 1, M < 1, ptr not starting at 0 / decreasing, species out of range, sigma < 1, v = 0,
+ * a species twice in one row, v_jk < -sigma_jk, rate negative / NaN / inf) or RT_ERR_UNSUPPORTED. */
+int rt_validate_network(const rt_network *net);
+
+/* Validate, build the species->reactions dependency lists (Gibson & Bruck's dependency graph,
+ * PAPER.md:191, stored two-hop: stoich row of mu -> species -> reactions reading that species)
+ * and deep-copy everything to `device`.  *out receives the model. */
+int rt_create(const rt_network *net, int device, rt_model **out);
+
+/* One trajectory (Table 3 loop).  Runs until max_firings reactions have fired
+ * (0 = no firing limit), until the next firing would pass t_end (+inf = no time limit; at least
+ * one limit is required), or until absorbed.
+ *   x0 [N] initial counts; x_out [N] final counts (may alias nothing; may be NULL).
+ *   res: outcome (required).
+ *   fire_count_out [M] firings per reaction R_k (Eq.5), T_out/P_out [M] final internal times and
+ *   next internal firing times -- each may be NULL.
+ *   trace_mu/trace_t [trace_cap]: the fired reaction and the time of each of the first trace_cap
+ *   firings (either may be NULL; trace_cap may be 0).
+ * Returns RT_ERR_OVERFLOW (also in res->status) if a count left the bound; outputs then hold the
+ * state at the offending firing. */
+int rt_run(rt_model *m, const int64_t *x0, uint64_t seed, uint64_t trajectory,
+           uint64_t max_firings, double t_end,
+           int64_t *x_out, rt_result *res,
+           uint64_t *fire_count_out, double *T_out, double *P_out,
+           int32_t *trace_mu, double *trace_t, uint64_t trace_cap);
+
+/* Same trajectory, with x0 / x_out / trace_* DEVICE pointers on m's device and the work
+ * enqueued on `stream` (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream; NULL = the
+ * default stream).  res_dev: device pointer to one rt_result.  The call does not synchronise;
+ * device-side failures (overflow, barrier timeout) are reported in res_dev->status and by the
+ * next rt_sync.  x_out_dev, trace_*_dev may be NULL. */
+int rt_run_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t trajectory,
+               uint64_t max_firings, double t_end,
+               int64_t *x_out_dev, rt_result *res_dev,
+               int32_t *trace_mu_dev, double *trace_t_dev, uint64_t trace_cap, void *stream);
+
+/* n_traj independent trajectories traj_first .. traj_first+n_traj-1 from the same x0 (the
+ * paper's "bundles").  Row i of the outputs is exactly what
+ * rt_run(trajectory = traj_first + i) returns.  x_out [n_traj*N] row-major (may be NULL),
+ * res [n_traj].  Returns the first non-OK per-trajectory status, if any. */
+int rt_ensemble(rt_model *m, const int64_t *x0, uint64_t seed, uint64_t traj_first,
+                uint64_t n_traj, uint64_t max_firings, double t_end,
+                int64_t *x_out, rt_result *res);
+
+/* Device-pointer flavour of rt_ensemble (x0_dev [N], x_out_dev [n_traj*N] or NULL,
+ * res_dev [n_traj]), enqueued on `stream`, no synchronisation. */
+int rt_ensemble_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t traj_first,
+                    uint64_t n_traj, uint64_t max_firings, double t_end,
+                    int64_t *x_out_dev, rt_result *res_dev, void *stream);
+
+/* Wait for everything enqueued on `stream` by this model; returns RT_ERR_CUDA if a kernel
+ * reported a barrier timeout or the runtime reported an error. */
+int rt_sync(rt_model *m, void *stream);
+
+/* Tuning / debug knobs (all optional; results never depend on them).
+ *   "refresh_mode"   0 = dependency-graph refresh of a_k (default), 1 = recompute every a_k
+ *                    each firing (the paper's own GPU scheme)
+ *   "bundle_ctas"    CTAs cooperating on one trajectory; 0 = choose automatically
+ *   "ensemble_path"  0 = automatic, 1 = force one-thread-per-trajectory kernel,
+ *                    2 = force the bundle (CTA-group-per-trajectory) kernel
+ * Returns RT_ERR_BAD_ARG for an unknown name or value. */
+int rt_set_option(rt_model *m, const char *name, int64_t value);
+
+/* Introspection for tests and bench.py:
+ *   "kernel_launches"  kernels launched by this model so far
+ *   "bundle_ctas", "bundles", "block_threads"  shape of the last bundle launch
+ *   "ensemble_path"    path taken by the last rt_ensemble call (1 or 2)
+ *   "num_sms", "dep_entries", "max_sigma"
+ * Unknown name: returns RT_ERR_BAD_ARG and leaves *value alone. */
+int rt_get_info(const rt_model *m, const char *name, int64_t *value);
+
+void rt_destroy(rt_model *m);            /* rt_destroy(NULL) is a no-op */
+
+const char *rt_strerror(int code);       /* static string, never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RT_B200_H_ */

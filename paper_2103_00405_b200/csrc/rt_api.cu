@@ -1,0 +1,495 @@
+// rt_api.cu -- host side of the C ABI declared in include/rt.h: validation, dependency-list
+// construction, device store, launch planning.  Every step of the simulation itself runs in the
+// kernels of rt_bundle.cuh / rt_thread.cuh; there is no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/rt.h"
+#include "rt_bundle.cuh"
+#include "rt_thread.cuh"
+
+using rt::u64;
+
+namespace {
+
+constexpr int kBlock = 1024;          // threads per CTA of the bundle kernel
+constexpr int kThreadKernelMaxM = 64; // one-thread-per-trajectory path: M, N at most this
+constexpr int kMinPairsPerCta = 256;  // do not spread a trajectory thinner than this
+
+#define CU_TRY(expr)                                                         \
+  do {                                                                       \
+    cudaError_t e_ = (expr);                                                 \
+    if (e_ != cudaSuccess) {                                                 \
+      if (getenv("RT_DEBUG"))                                                \
+        fprintf(stderr, "rt: %s -> %s\n", #expr, cudaGetErrorString(e_));    \
+      return e_ == cudaErrorMemoryAllocation ? RT_ERR_OOM : RT_ERR_CUDA;     \
+    }                                                                        \
+  } while (0)
+
+struct DevBuf {
+  void *p = nullptr;
+  size_t bytes = 0;
+  int ensure(size_t want) {
+    if (want <= bytes) return RT_OK;
+    if (p) cudaFree(p);
+    p = nullptr;
+    bytes = 0;
+    cudaError_t e = cudaMalloc(&p, want);
+    if (e != cudaSuccess) { p = nullptr; return e == cudaErrorMemoryAllocation ? RT_ERR_OOM : RT_ERR_CUDA; }
+    bytes = want;
+    return RT_OK;
+  }
+  void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
+};
+
+}  // namespace
+
+struct rt_model {
+  int device = 0;
+  int num_sms = 0;
+  rt::NetDev net{};
+  uint32_t nnz_r = 0, nnz_v = 0;
+  int max_sigma = 1;
+  // device copies of the network
+  DevBuf d_react_ptr, d_react_species, d_react_sigma, d_stoich_ptr, d_stoich_species, d_stoich_v,
+      d_rate, d_dep_ptr, d_dep_rxn;
+  // per-bundle state
+  DevBuf d_T, d_P, d_a, d_n, d_X, d_exch, d_xgen, d_err;
+  // staging for the host-pointer API
+  DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t;
+  // options
+  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0;
+  // info
+  int64_t kernel_launches = 0;
+  int last_S = 0, last_B = 0, last_path = 0;
+};
+
+namespace {
+
+int validate(const rt_network *net, int *max_sigma_out) {
+  if (!net) return RT_ERR_NULL;
+  if (!net->react_ptr || !net->stoich_ptr || !net->rate) return RT_ERR_NULL;
+  const int64_t N = net->n_species, M = net->n_reactions;
+  if (N < 1 || M < 1) return RT_ERR_BAD_NETWORK;
+  if (net->react_ptr[0] != 0 || net->stoich_ptr[0] != 0) return RT_ERR_BAD_NETWORK;
+  for (int64_t k = 0; k < M; ++k)
+    if (net->react_ptr[k + 1] < net->react_ptr[k] || net->stoich_ptr[k + 1] < net->stoich_ptr[k])
+      return RT_ERR_BAD_NETWORK;
+  const int64_t nr = net->react_ptr[M], nv = net->stoich_ptr[M];
+  if ((nr > 0 && (!net->react_species || !net->react_sigma)) ||
+      (nv > 0 && (!net->stoich_species || !net->stoich_v)))
+    return RT_ERR_NULL;
+  if (nr >= (int64_t)0xffffffffll || nv >= (int64_t)0xffffffffll) return RT_ERR_UNSUPPORTED;
+  int max_sigma = 1;
+  bool unsupported = false;
+  std::vector<int32_t> row;
+  for (int64_t k = 0; k < M; ++k) {
+    if (!std::isfinite(net->rate[k]) || net->rate[k] < 0.0) return RT_ERR_BAD_NETWORK;
+    const int64_t rb = net->react_ptr[k], re = net->react_ptr[k + 1];
+    for (int64_t e = rb; e < re; ++e) {
+      const int32_t j = net->react_species[e], s = net->react_sigma[e];
+      if (j < 0 || j >= N || s < 1) return RT_ERR_BAD_NETWORK;
+      if (s > 3) unsupported = true;
+      max_sigma = std::max(max_sigma, (int)std::min(s, 4));
+      for (int64_t f = rb; f < e; ++f)
+        if (net->react_species[f] == j) return RT_ERR_BAD_NETWORK;     // G18: A+A must be sigma=2
+    }
+    const int64_t sb = net->stoich_ptr[k], se = net->stoich_ptr[k + 1];
+    for (int64_t e = sb; e < se; ++e) {
+      const int32_t j = net->stoich_species[e], v = net->stoich_v[e];
+      if (j < 0 || j >= N || v == 0) return RT_ERR_BAD_NETWORK;
+      for (int64_t f = sb; f < e; ++f)
+        if (net->stoich_species[f] == j) return RT_ERR_BAD_NETWORK;
+      if (v < 0) {   // may not remove more than the reaction requires
+        int32_t sigma = 0;
+        for (int64_t f = rb; f < re; ++f)
+          if (net->react_species[f] == j) sigma = net->react_sigma[f];
+        if ((int64_t)v < -(int64_t)sigma) return RT_ERR_BAD_NETWORK;
+      }
+    }
+  }
+  if (unsupported) return RT_ERR_UNSUPPORTED;
+  if (max_sigma_out) *max_sigma_out = max_sigma;
+  return RT_OK;
+}
+
+template <typename T>
+int upload(DevBuf &buf, const std::vector<T> &host) {
+  const size_t bytes = std::max<size_t>(host.size() * sizeof(T), 16);
+  int rc = buf.ensure(bytes);
+  if (rc != RT_OK) return rc;
+  if (!host.empty()) CU_TRY(cudaMemcpy(buf.p, host.data(), host.size() * sizeof(T), cudaMemcpyHostToDevice));
+  return RT_OK;
+}
+
+// How one launch is shaped: B bundles of S CTAs.
+struct Plan { int S, B; int pairs_per_cta; };
+
+Plan plan_bundles(const rt_model *m, u64 n_traj) {
+  const int pairs_total = m->net.M_pad / 2;
+  const int sms = m->num_sms;
+  int S;
+  if (m->opt_bundle_ctas > 0) {
+    S = std::min(m->opt_bundle_ctas, sms);
+  } else if (n_traj <= 1) {
+    S = sms;                                            // one trajectory: the whole chip
+  } else {
+    S = (int)std::max<u64>(1, (u64)sms / n_traj);       // many: as many bundles as fit
+  }
+  S = std::min(S, std::max(1, (pairs_total + kMinPairsPerCta - 1) / kMinPairsPerCta));
+  S = std::max(S, 1);
+  Plan pl;
+  pl.S = S;
+  pl.B = (int)std::min<u64>(std::max<u64>(n_traj, 1), (u64)(sms / S));
+  pl.pairs_per_cta = (pairs_total + S - 1) / S;
+  return pl;
+}
+
+int ensure_state(rt_model *m, const Plan &pl) {
+  const size_t Mp = (size_t)m->net.M_pad, N = (size_t)m->net.N, B = (size_t)pl.B;
+  int rc;
+  if ((rc = m->d_T.ensure(B * Mp * 8)) != RT_OK) return rc;
+  if ((rc = m->d_P.ensure(B * Mp * 8)) != RT_OK) return rc;
+  if ((rc = m->d_a.ensure(B * Mp * 8)) != RT_OK) return rc;
+  if ((rc = m->d_n.ensure(B * Mp * 4)) != RT_OK) return rc;
+  if ((rc = m->d_X.ensure(B * N * 8)) != RT_OK) return rc;
+  if ((rc = m->d_exch.ensure(B * 2 * (size_t)pl.S * 2 * 8)) != RT_OK) return rc;
+  if ((rc = m->d_xgen.ensure(B * 32 * 4)) != RT_OK) return rc;
+  if ((rc = m->d_err.ensure(16)) != RT_OK) return rc;
+  return RT_OK;
+}
+
+int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_first, u64 n_traj,
+                   u64 max_firings, double t_end, long long *x_out_dev, rt_result *res_dev,
+                   int32_t *trace_mu_dev, double *trace_t_dev, u64 trace_cap, cudaStream_t st) {
+  const Plan pl = plan_bundles(m, n_traj);
+  int rc = ensure_state(m, pl);
+  if (rc != RT_OK) return rc;
+  CU_TRY(cudaMemsetAsync(m->d_exch.p, 0, (size_t)pl.B * 2 * pl.S * 2 * 8, st));
+  CU_TRY(cudaMemsetAsync(m->d_xgen.p, 0, (size_t)pl.B * 32 * 4, st));
+  rt::BundleParams p{};
+  p.net = m->net;
+  p.T = (double *)m->d_T.p; p.P = (double *)m->d_P.p; p.a = (double *)m->d_a.p;
+  p.n = (uint32_t *)m->d_n.p; p.X = (long long *)m->d_X.p;
+  p.exch = (u64 *)m->d_exch.p; p.xgen = (uint32_t *)m->d_xgen.p;
+  p.S = pl.S; p.B = pl.B; p.pairs_per_cta = pl.pairs_per_cta;
+  p.x0 = x0_dev; p.seed = seed; p.traj_first = traj_first; p.n_traj = n_traj;
+  p.max_firings = max_firings; p.t_end = t_end;
+  p.x_out = x_out_dev; p.res = res_dev;
+  p.trace_mu = trace_mu_dev; p.trace_t = trace_t_dev;
+  p.trace_cap = (trace_mu_dev || trace_t_dev) ? trace_cap : 0;
+  p.refresh_mode = m->refresh_mode;
+  p.err = (int *)m->d_err.p;
+  void *args[] = {&p};
+  // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
+  CU_TRY(cudaLaunchCooperativeKernel((const void *)rt::rt_bundle_kernel<kBlock>, dim3(pl.S * pl.B),
+                                     dim3(kBlock), args, 0, st));
+  m->kernel_launches += 1;
+  m->last_S = pl.S; m->last_B = pl.B; m->last_path = 2;
+  return RT_OK;
+}
+
+template <int BLOCK>
+int launch_thread_kernel(rt_model *m, const rt::ThreadParams &p, size_t smem, cudaStream_t st) {
+  CU_TRY(cudaFuncSetAttribute(rt::rt_thread_kernel<BLOCK>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)smem));
+  const unsigned grid = (unsigned)((p.n_traj + BLOCK - 1) / BLOCK);
+  rt::rt_thread_kernel<BLOCK><<<grid, BLOCK, smem, st>>>(p);
+  CU_TRY(cudaGetLastError());
+  m->kernel_launches += 1;
+  m->last_path = 1;
+  return RT_OK;
+}
+
+bool thread_path_fits(const rt_model *m) {
+  return m->net.M <= kThreadKernelMaxM && m->net.N <= kThreadKernelMaxM &&
+         rt::thread_kernel_smem(m->net.M, m->net.N, m->nnz_r, m->nnz_v, 32) <= 200 * 1024;
+}
+
+int launch_threads(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_first, u64 n_traj,
+                   u64 max_firings, double t_end, long long *x_out_dev, rt_result *res_dev,
+                   cudaStream_t st) {
+  rt::ThreadParams p{};
+  p.net = m->net; p.nnz_r = m->nnz_r; p.nnz_v = m->nnz_v;
+  p.x0 = x0_dev; p.seed = seed; p.traj_first = traj_first; p.n_traj = n_traj;
+  p.max_firings = max_firings; p.t_end = t_end; p.x_out = x_out_dev; p.res = res_dev;
+  // Smallest CTA that still fills the chip: more CTAs -> finer balance over the 148 SMs.
+  const size_t s32 = rt::thread_kernel_smem(m->net.M, m->net.N, m->nnz_r, m->nnz_v, 32);
+  const size_t s128 = rt::thread_kernel_smem(m->net.M, m->net.N, m->nnz_r, m->nnz_v, 128);
+  if (n_traj >= (u64)m->num_sms * 2048 && s128 <= 48 * 1024)
+    return launch_thread_kernel<128>(m, p, s128, st);
+  return launch_thread_kernel<32>(m, p, s32, st);
+}
+
+int check_limits(u64 max_firings, double t_end) {
+  if (std::isnan(t_end) || t_end < 0.0) return RT_ERR_BAD_ARG;
+  if (max_firings == 0 && std::isinf(t_end)) return RT_ERR_BAD_ARG;
+  return RT_OK;
+}
+
+int check_x0(const rt_model *m, const int64_t *x0) {
+  for (int32_t j = 0; j < m->net.N; ++j)
+    if (x0[j] < 0 || x0[j] > m->net.xmax) return RT_ERR_BAD_ARG;
+  return RT_OK;
+}
+
+int finish(rt_model *m, cudaStream_t st) {
+  CU_TRY(cudaStreamSynchronize(st));
+  if (m->d_err.p) {
+    int err = 0;
+    CU_TRY(cudaMemcpy(&err, m->d_err.p, sizeof(int), cudaMemcpyDeviceToHost));
+    if (err) { cudaMemset(m->d_err.p, 0, sizeof(int)); return RT_ERR_CUDA; }
+  }
+  return RT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rt_validate_network(const rt_network *net) { return validate(net, nullptr); }
+
+int rt_create(const rt_network *net, int device, rt_model **out) {
+  if (!out) return RT_ERR_NULL;
+  *out = nullptr;
+  int max_sigma = 1;
+  int rc = validate(net, &max_sigma);
+  if (rc != RT_OK) return rc;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev) {
+    cudaGetLastError();
+    return RT_ERR_CUDA;
+  }
+  CU_TRY(cudaSetDevice(device));
+  rt_model *m = new (std::nothrow) rt_model();
+  if (!m) return RT_ERR_OOM;
+  m->device = device;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { delete m; return RT_ERR_CUDA; }
+  m->num_sms = prop.multiProcessorCount;
+  if (!prop.cooperativeLaunch) { delete m; return RT_ERR_CUDA; }
+
+  const int32_t N = net->n_species, M = net->n_reactions;
+  const size_t nr = (size_t)net->react_ptr[M], nv = (size_t)net->stoich_ptr[M];
+  std::vector<uint32_t> rp(M + 1), sp(M + 1);
+  for (int32_t k = 0; k <= M; ++k) { rp[k] = (uint32_t)net->react_ptr[k]; sp[k] = (uint32_t)net->stoich_ptr[k]; }
+  std::vector<int32_t> rs(net->react_species, net->react_species + nr),
+      rg(net->react_sigma, net->react_sigma + nr), ss(net->stoich_species, net->stoich_species + nv),
+      sv(net->stoich_v, net->stoich_v + nv);
+  std::vector<double> rate(net->rate, net->rate + M);
+  // dependency lists: species j -> reactions with j as a reactant, ascending reaction index
+  // (counting sort over the reactant CSR, which is already ordered by reaction).
+  std::vector<uint32_t> dp((size_t)N + 1, 0u);
+  for (size_t e = 0; e < nr; ++e) dp[(size_t)rs[e] + 1] += 1u;
+  for (int32_t j = 0; j < N; ++j) dp[j + 1] += dp[j];
+  std::vector<int32_t> dr(nr);
+  {
+    std::vector<uint32_t> cursor(dp.begin(), dp.end() - 1);
+    for (int32_t k = 0; k < M; ++k)
+      for (uint32_t e = rp[k]; e < rp[k + 1]; ++e) dr[cursor[rs[e]]++] = k;
+  }
+  rc = RT_OK;
+  if (rc == RT_OK) rc = upload(m->d_react_ptr, rp);
+  if (rc == RT_OK) rc = upload(m->d_react_species, rs);
+  if (rc == RT_OK) rc = upload(m->d_react_sigma, rg);
+  if (rc == RT_OK) rc = upload(m->d_stoich_ptr, sp);
+  if (rc == RT_OK) rc = upload(m->d_stoich_species, ss);
+  if (rc == RT_OK) rc = upload(m->d_stoich_v, sv);
+  if (rc == RT_OK) rc = upload(m->d_rate, rate);
+  if (rc == RT_OK) rc = upload(m->d_dep_ptr, dp);
+  if (rc == RT_OK) rc = upload(m->d_dep_rxn, dr);
+  if (rc == RT_OK) rc = m->d_err.ensure(16);
+  if (rc == RT_OK && cudaMemset(m->d_err.p, 0, 16) != cudaSuccess) rc = RT_ERR_CUDA;
+  if (rc != RT_OK) { rt_destroy(m); return rc; }
+
+  m->nnz_r = (uint32_t)nr; m->nnz_v = (uint32_t)nv; m->max_sigma = max_sigma;
+  rt::NetDev &d = m->net;
+  d.N = N; d.M = M; d.M_pad = (M + 1) & ~1;
+  d.react_ptr = (const uint32_t *)m->d_react_ptr.p;
+  d.react_species = (const int32_t *)m->d_react_species.p;
+  d.react_sigma = (const int32_t *)m->d_react_sigma.p;
+  d.stoich_ptr = (const uint32_t *)m->d_stoich_ptr.p;
+  d.stoich_species = (const int32_t *)m->d_stoich_species.p;
+  d.stoich_v = (const int32_t *)m->d_stoich_v.p;
+  d.rate = (const double *)m->d_rate.p;
+  d.dep_ptr = (const uint32_t *)m->d_dep_ptr.p;
+  d.dep_rxn = (const int32_t *)m->d_dep_rxn.p;
+  d.xmax = max_sigma <= 2 ? ((1ll << 31) - 1) : ((1ll << 21) - 1);
+  *out = m;
+  return RT_OK;
+}
+
+int rt_run_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t trajectory,
+               uint64_t max_firings, double t_end, int64_t *x_out_dev, rt_result *res_dev,
+               int32_t *trace_mu_dev, double *trace_t_dev, uint64_t trace_cap, void *stream) {
+  if (!m || !x0_dev || !res_dev) return RT_ERR_NULL;
+  int rc = check_limits(max_firings, t_end);
+  if (rc != RT_OK) return rc;
+  CU_TRY(cudaSetDevice(m->device));
+  return launch_bundles(m, (const long long *)x0_dev, seed, trajectory, 1, max_firings, t_end,
+                        (long long *)x_out_dev, res_dev, trace_mu_dev, trace_t_dev, trace_cap,
+                        (cudaStream_t)stream);
+}
+
+int rt_run(rt_model *m, const int64_t *x0, uint64_t seed, uint64_t trajectory,
+           uint64_t max_firings, double t_end, int64_t *x_out, rt_result *res,
+           uint64_t *fire_count_out, double *T_out, double *P_out,
+           int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
+  if (!m || !x0 || !res) return RT_ERR_NULL;
+  int rc = check_limits(max_firings, t_end);
+  if (rc != RT_OK) return rc;
+  if ((rc = check_x0(m, x0)) != RT_OK) return rc;
+  CU_TRY(cudaSetDevice(m->device));
+  const size_t N = (size_t)m->net.N, M = (size_t)m->net.M;
+  if (!trace_mu && !trace_t) trace_cap = 0;
+  if ((rc = m->d_x0.ensure(N * 8)) != RT_OK) return rc;
+  if ((rc = m->d_xout.ensure(N * 8)) != RT_OK) return rc;
+  if ((rc = m->d_res.ensure(sizeof(rt_result))) != RT_OK) return rc;
+  if (trace_cap) {
+    if ((rc = m->d_trace_mu.ensure(trace_cap * 4)) != RT_OK) return rc;
+    if ((rc = m->d_trace_t.ensure(trace_cap * 8)) != RT_OK) return rc;
+  }
+  cudaStream_t st = 0;
+  CU_TRY(cudaMemcpyAsync(m->d_x0.p, x0, N * 8, cudaMemcpyHostToDevice, st));
+  CU_TRY(cudaMemsetAsync(m->d_res.p, 0, sizeof(rt_result), st));
+  rc = launch_bundles(m, (const long long *)m->d_x0.p, seed, trajectory, 1, max_firings, t_end,
+                      (long long *)m->d_xout.p, (rt_result *)m->d_res.p,
+                      trace_cap ? (int32_t *)m->d_trace_mu.p : nullptr,
+                      trace_cap ? (double *)m->d_trace_t.p : nullptr, trace_cap, st);
+  if (rc != RT_OK) return rc;
+  if ((rc = finish(m, st)) != RT_OK) return rc;
+  CU_TRY(cudaMemcpy(res, m->d_res.p, sizeof(rt_result), cudaMemcpyDeviceToHost));
+  if (x_out) CU_TRY(cudaMemcpy(x_out, m->d_xout.p, N * 8, cudaMemcpyDeviceToHost));
+  const size_t nrec = (size_t)std::min<uint64_t>(res->firings, trace_cap);
+  if (trace_mu && nrec) CU_TRY(cudaMemcpy(trace_mu, m->d_trace_mu.p, nrec * 4, cudaMemcpyDeviceToHost));
+  if (trace_t && nrec) CU_TRY(cudaMemcpy(trace_t, m->d_trace_t.p, nrec * 8, cudaMemcpyDeviceToHost));
+  if (T_out) CU_TRY(cudaMemcpy(T_out, m->d_T.p, M * 8, cudaMemcpyDeviceToHost));
+  if (P_out) CU_TRY(cudaMemcpy(P_out, m->d_P.p, M * 8, cudaMemcpyDeviceToHost));
+  if (fire_count_out) {
+    std::vector<uint32_t> n32(M);
+    CU_TRY(cudaMemcpy(n32.data(), m->d_n.p, M * 4, cudaMemcpyDeviceToHost));
+    for (size_t k = 0; k < M; ++k) fire_count_out[k] = n32[k];
+  }
+  return res->status;
+}
+
+int rt_ensemble_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t traj_first,
+                    uint64_t n_traj, uint64_t max_firings, double t_end, int64_t *x_out_dev,
+                    rt_result *res_dev, void *stream) {
+  if (!m || !x0_dev || !res_dev) return RT_ERR_NULL;
+  int rc = check_limits(max_firings, t_end);
+  if (rc != RT_OK) return rc;
+  if (n_traj == 0) return RT_OK;
+  CU_TRY(cudaSetDevice(m->device));
+  bool use_threads = thread_path_fits(m);
+  if (m->opt_ensemble_path == 1) {
+    if (!thread_path_fits(m)) return RT_ERR_BAD_ARG;
+    use_threads = true;
+  } else if (m->opt_ensemble_path == 2) {
+    use_threads = false;
+  }
+  if (use_threads)
+    return launch_threads(m, (const long long *)x0_dev, seed, traj_first, n_traj, max_firings, t_end,
+                          (long long *)x_out_dev, res_dev, (cudaStream_t)stream);
+  return launch_bundles(m, (const long long *)x0_dev, seed, traj_first, n_traj, max_firings, t_end,
+                        (long long *)x_out_dev, res_dev, nullptr, nullptr, 0, (cudaStream_t)stream);
+}
+
+int rt_ensemble(rt_model *m, const int64_t *x0, uint64_t seed, uint64_t traj_first,
+                uint64_t n_traj, uint64_t max_firings, double t_end, int64_t *x_out,
+                rt_result *res) {
+  if (!m || !x0 || !res) return RT_ERR_NULL;
+  int rc = check_limits(max_firings, t_end);
+  if (rc != RT_OK) return rc;
+  if ((rc = check_x0(m, x0)) != RT_OK) return rc;
+  if (n_traj == 0) return RT_OK;
+  CU_TRY(cudaSetDevice(m->device));
+  const size_t N = (size_t)m->net.N;
+  if ((rc = m->d_x0.ensure(N * 8)) != RT_OK) return rc;
+  if ((rc = m->d_res.ensure(n_traj * sizeof(rt_result))) != RT_OK) return rc;
+  if (x_out && (rc = m->d_xout.ensure(n_traj * N * 8)) != RT_OK) return rc;
+  cudaStream_t st = 0;
+  CU_TRY(cudaMemcpyAsync(m->d_x0.p, x0, N * 8, cudaMemcpyHostToDevice, st));
+  CU_TRY(cudaMemsetAsync(m->d_res.p, 0, n_traj * sizeof(rt_result), st));
+  rc = rt_ensemble_dev(m, (const int64_t *)m->d_x0.p, seed, traj_first, n_traj, max_firings, t_end,
+                       x_out ? (int64_t *)m->d_xout.p : nullptr, (rt_result *)m->d_res.p, st);
+  if (rc != RT_OK) return rc;
+  if ((rc = finish(m, st)) != RT_OK) return rc;
+  CU_TRY(cudaMemcpy(res, m->d_res.p, n_traj * sizeof(rt_result), cudaMemcpyDeviceToHost));
+  if (x_out) CU_TRY(cudaMemcpy(x_out, m->d_xout.p, n_traj * N * 8, cudaMemcpyDeviceToHost));
+  for (uint64_t i = 0; i < n_traj; ++i)
+    if (res[i].status != RT_OK) return res[i].status;
+  return RT_OK;
+}
+
+int rt_sync(rt_model *m, void *stream) {
+  if (!m) return RT_ERR_NULL;
+  CU_TRY(cudaSetDevice(m->device));
+  return finish(m, (cudaStream_t)stream);
+}
+
+int rt_set_option(rt_model *m, const char *name, int64_t value) {
+  if (!m || !name) return RT_ERR_NULL;
+  if (!strcmp(name, "refresh_mode")) {
+    if (value != 0 && value != 1) return RT_ERR_BAD_ARG;
+    m->refresh_mode = (int)value;
+  } else if (!strcmp(name, "bundle_ctas")) {
+    if (value < 0 || value > 1024) return RT_ERR_BAD_ARG;
+    m->opt_bundle_ctas = (int)value;
+  } else if (!strcmp(name, "ensemble_path")) {
+    if (value < 0 || value > 2) return RT_ERR_BAD_ARG;
+    m->opt_ensemble_path = (int)value;
+  } else {
+    return RT_ERR_BAD_ARG;
+  }
+  return RT_OK;
+}
+
+int rt_get_info(const rt_model *m, const char *name, int64_t *value) {
+  if (!m || !name || !value) return RT_ERR_NULL;
+  if (!strcmp(name, "kernel_launches")) *value = m->kernel_launches;
+  else if (!strcmp(name, "bundle_ctas")) *value = m->last_S;
+  else if (!strcmp(name, "bundles")) *value = m->last_B;
+  else if (!strcmp(name, "block_threads")) *value = kBlock;
+  else if (!strcmp(name, "ensemble_path")) *value = m->last_path;
+  else if (!strcmp(name, "num_sms")) *value = m->num_sms;
+  else if (!strcmp(name, "dep_entries")) *value = m->nnz_r;
+  else if (!strcmp(name, "max_sigma")) *value = m->max_sigma;
+  else return RT_ERR_BAD_ARG;
+  return RT_OK;
+}
+
+void rt_destroy(rt_model *m) {
+  if (!m) return;
+  cudaSetDevice(m->device);
+  DevBuf *bufs[] = {&m->d_react_ptr, &m->d_react_species, &m->d_react_sigma, &m->d_stoich_ptr,
+                    &m->d_stoich_species, &m->d_stoich_v, &m->d_rate, &m->d_dep_ptr, &m->d_dep_rxn,
+                    &m->d_T, &m->d_P, &m->d_a, &m->d_n, &m->d_X, &m->d_exch, &m->d_xgen, &m->d_err,
+                    &m->d_x0, &m->d_xout, &m->d_res, &m->d_trace_mu, &m->d_trace_t};
+  for (DevBuf *b : bufs) b->release();
+  delete m;
+}
+
+const char *rt_strerror(int code) {
+  switch (code) {
+    case RT_OK: return "ok";
+    case RT_ERR_NULL: return "null pointer argument";
+    case RT_ERR_BAD_NETWORK: return "invalid reaction network";
+    case RT_ERR_BAD_ARG: return "invalid argument";
+    case RT_ERR_UNSUPPORTED: return "unsupported network (sigma > 3 or too many entries)";
+    case RT_ERR_OVERFLOW: return "species count left the supported range";
+    case RT_ERR_CUDA: return "CUDA error or in-kernel barrier timeout";
+    case RT_ERR_OOM: return "out of memory";
+    default: return "unknown error code";
+  }
+}
+
+}  // extern "C"

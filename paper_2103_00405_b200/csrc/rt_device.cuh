@@ -1,0 +1,126 @@
+// rt_device.cuh -- device-side building blocks shared by the sm_100a kernels of this library.
+// (Nothing here is shared with oracle/: the oracle has its own Philox, draw and propensity.)
+//
+// All fp64 arithmetic that decides a result uses the rounding-explicit intrinsics
+// (__dmul_rn / __dadd_rn / __dsub_rn / __ddiv_rn), which nvcc never contracts into FMAs, so
+// every operation is one IEEE round-to-nearest step in the order DESIGN.md fixes.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace rt {
+
+typedef unsigned long long u64;
+
+// Device copy of the network (rt_network of include/rt.h) plus the dependency lists.
+struct NetDev {
+  int32_t N, M;
+  int32_t M_pad;                 // M rounded up to even; entry M (if any) has a = 0, T = P = 0
+  const uint32_t *react_ptr;     // [M+1]
+  const int32_t *react_species;  // [nnz_r]
+  const int32_t *react_sigma;    // [nnz_r]
+  const uint32_t *stoich_ptr;    // [M+1]
+  const int32_t *stoich_species; // [nnz_v]
+  const int32_t *stoich_v;       // [nnz_v]
+  const double *rate;            // [M]
+  const uint32_t *dep_ptr;       // [N+1]  species j -> reactions that have j as a reactant
+  const int32_t *dep_rxn;        // [nnz_r] sorted by reaction index within a species
+  long long xmax;                // count bound (2^31-1, or 2^21-1 if some sigma = 3)
+};
+
+// ------------------------------------------------------------------ Philox4x32-10
+// Salmon et al., SC'11.  Returns output words 0 and 1 (the two the draw uses).
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1,
+                                              uint32_t &o0, uint32_t &o1) {
+#pragma unroll
+  for (int i = 0; i < 10; ++i) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    c0 = hi1 ^ c1 ^ k0;
+    c1 = lo1;
+    c2 = hi0 ^ c3 ^ k1;
+    c3 = lo0;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  o0 = c0;
+  o1 = c1;
+}
+
+// n-th unit-exponential increment of channel k (Eq.23: Delta T = ln(1/r)).
+// key = (lo32 seed, hi32 seed), counter = (k, n, lo32 traj, hi32 traj);
+// r = (u53 + 1) * 2^-53 in (0, 1].
+__device__ __forceinline__ double exp_draw(u64 seed, u64 traj, uint32_t k, uint32_t n) {
+  uint32_t w0, w1;
+  philox4x32_10(k, n, (uint32_t)traj, (uint32_t)(traj >> 32), (uint32_t)seed,
+                (uint32_t)(seed >> 32), w0, w1);
+  const u64 u53 = (((u64)w1 << 32) | (u64)w0) >> 11;
+  const double r = __dmul_rn(__ull2double_rn(u53 + 1ull), 0x1.0p-53);
+  return -log(r);
+}
+
+// C(x, sigma), exact integer (Eq.2; reading G2).
+__device__ __forceinline__ long long binom(long long x, int sigma) {
+  if (sigma == 1) return x;
+  const long long h = x * (x - 1) / 2;
+  if (sigma == 2) return h;
+  return h * (x - 2) / 3;
+}
+
+// a_k = c_k * prod_j C(X_j, sigma_jk): one rounded multiply per reactant, CSR order.
+// X is read with ld.global.cg (L2): another CTA may have written it since this SM's L1 saw it.
+__device__ __forceinline__ double propensity(const NetDev &net, const long long *X, int k) {
+  double a = __ldg(net.rate + k);
+  const uint32_t e1 = __ldg(net.react_ptr + k + 1);
+  for (uint32_t e = __ldg(net.react_ptr + k); e < e1; ++e) {
+    const long long x = __ldcg(X + __ldg(net.react_species + e));
+    a = __dmul_rn(a, __ll2double_rn(binom(x, __ldg(net.react_sigma + e))));
+  }
+  return a;
+}
+
+// ------------------------------------------------------------------ lexicographic argmin
+struct Cand {
+  double dt;
+  int k;
+};
+__device__ __forceinline__ bool cand_less(double dt, int k, const Cand &b) {
+  return dt < b.dt || (dt == b.dt && k < b.k);
+}
+__device__ __forceinline__ Cand warp_lexmin(Cand c) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    const double odt = __shfl_xor_sync(0xffffffffu, c.dt, off);
+    const int ok = __shfl_xor_sync(0xffffffffu, c.k, off);
+    if (cand_less(odt, ok, c)) { c.dt = odt; c.k = ok; }
+  }
+  return c;
+}
+
+// Waiting time of one channel (Eq.24 with constant a_k; readings G4, G7): a <= 0 (which
+// includes "flagged for refresh", stored as -|a|, and a = -0.0) gives +inf.
+__device__ __forceinline__ double waiting_time(double P, double T, double a) {
+  if (!(a > 0.0)) return __longlong_as_double(0x7ff0000000000000ll);
+  double r = __dsub_rn(P, T);
+  r = r < 0.0 ? 0.0 : r;
+  return __ddiv_rn(r, a);
+}
+
+// ------------------------------------------------------------------ memory-model helpers
+__device__ __forceinline__ void st_release_u32(uint32_t *p, uint32_t v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_relaxed_v2(u64 *p, u64 a, u64 b) {
+  asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
+}
+__device__ __forceinline__ void ld_relaxed_v2(const u64 *p, u64 &a, u64 &b) {
+  asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+}
+
+}  // namespace rt

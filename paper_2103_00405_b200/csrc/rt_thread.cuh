@@ -1,0 +1,124 @@
+// rt_thread.cuh -- ensemble kernel for small networks: ONE THREAD = ONE TRAJECTORY
+// (north_star subsystem 5; the paper's Fig.1 workload is exactly this regime: 10 000 Lotka
+// trajectories side by side).  The network (a few CSR rows) is staged once per
+// CTA in shared memory; every thread keeps its whole state (T, P, a, n per reaction, X per
+// species) in shared memory, laid out [item][thread] so that a warp's accesses to item i hit
+// 32 different banks.  No thread ever talks to another: each lane loops over its own firings
+// to its own t_end / max_firings.  Every propensity is recomputed each firing (M is tiny), in
+// exactly the operation order of the bundle kernel, so the two paths give identical results.
+#pragma once
+#include "rt_device.cuh"
+#include "../../include/rt.h"
+
+namespace rt {
+
+struct ThreadParams {
+  NetDev net;
+  uint32_t nnz_r, nnz_v;
+  const long long *x0;
+  u64 seed, traj_first, n_traj, max_firings;
+  double t_end;
+  long long *x_out;      // [n_traj][N] or nullptr
+  rt_result *res;        // [n_traj]
+};
+
+// Shared-memory bytes: network copy + BLOCK * (3*8*M + 4*M + 8*N).
+__host__ __device__ inline size_t thread_kernel_smem(int M, int N, uint32_t nnz_r, uint32_t nnz_v,
+                                                     int block) {
+  size_t net = (size_t)M * 8 + 2 * (size_t)(M + 1) * 4 + 2 * (size_t)nnz_r * 4 + 2 * (size_t)nnz_v * 4;
+  net = (net + 15) & ~(size_t)15;
+  return net + (size_t)block * ((size_t)M * 28 + (size_t)N * 8);
+}
+
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK) rt_thread_kernel(const ThreadParams p) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const NetDev &net = p.net;
+  const int M = net.M, N = net.N, tid = threadIdx.x;
+  const double INF = __longlong_as_double(0x7ff0000000000000ll);
+
+  // ---- carve shared memory: network first, then per-thread state [item][BLOCK]
+  double *s_rate = reinterpret_cast<double *>(smem);
+  uint32_t *s_rp = reinterpret_cast<uint32_t *>(s_rate + M);
+  uint32_t *s_sp = s_rp + (M + 1);
+  int32_t *s_rs = reinterpret_cast<int32_t *>(s_sp + (M + 1));
+  int32_t *s_rg = s_rs + p.nnz_r;
+  int32_t *s_ss = s_rg + p.nnz_r;
+  int32_t *s_sv = s_ss + p.nnz_v;
+  size_t off = (size_t)M * 8 + 2 * (size_t)(M + 1) * 4 + 2 * (size_t)p.nnz_r * 4 + 2 * (size_t)p.nnz_v * 4;
+  off = (off + 15) & ~(size_t)15;
+  double *sT = reinterpret_cast<double *>(smem + off);
+  double *sP = sT + (size_t)M * BLOCK;
+  double *sA = sP + (size_t)M * BLOCK;
+  long long *sX = reinterpret_cast<long long *>(sA + (size_t)M * BLOCK);
+  uint32_t *sN = reinterpret_cast<uint32_t *>(sX + (size_t)N * BLOCK);
+
+  for (int i = tid; i < M; i += BLOCK) s_rate[i] = net.rate[i];
+  for (int i = tid; i <= M; i += BLOCK) { s_rp[i] = net.react_ptr[i]; s_sp[i] = net.stoich_ptr[i]; }
+  for (uint32_t i = tid; i < p.nnz_r; i += BLOCK) { s_rs[i] = net.react_species[i]; s_rg[i] = net.react_sigma[i]; }
+  for (uint32_t i = tid; i < p.nnz_v; i += BLOCK) { s_ss[i] = net.stoich_species[i]; s_sv[i] = net.stoich_v[i]; }
+  __syncthreads();
+
+  const u64 it = (u64)blockIdx.x * BLOCK + tid;
+  if (it >= p.n_traj) return;
+  const u64 traj = p.traj_first + it;
+
+#define ST(arr, i) arr[(size_t)(i) * BLOCK + tid]
+  for (int j = 0; j < N; ++j) ST(sX, j) = p.x0[j];
+  for (int k = 0; k < M; ++k) {
+    ST(sT, k) = 0.0;
+    ST(sP, k) = exp_draw(p.seed, traj, (uint32_t)k, 0u);
+    ST(sN, k) = 0u;
+  }
+  double t = 0.0;
+  u64 fired = 0;
+  int stop = 0, status = RT_OK;
+
+  for (;;) {
+    // a-1, a-2, a-3: propensities, waiting times, argmin (lowest k on ties: strict <, k ascending)
+    double delta = INF;
+    int mu = 0;
+    for (int k = 0; k < M; ++k) {
+      double a = s_rate[k];
+      for (uint32_t e = s_rp[k]; e < s_rp[k + 1]; ++e)
+        a = __dmul_rn(a, __ll2double_rn(binom(ST(sX, s_rs[e]), s_rg[e])));
+      ST(sA, k) = a;
+      const double d = waiting_time(ST(sP, k), ST(sT, k), a);
+      if (d < delta) { delta = d; mu = k; }
+    }
+    // a-4
+    if (delta == INF) { stop = RT_STOP_ABSORBED; break; }
+    if (p.t_end < INF && __dadd_rn(t, delta) > p.t_end) {
+      const double rest = __dsub_rn(p.t_end, t);
+      for (int k = 0; k < M; ++k) ST(sT, k) = __dadd_rn(ST(sT, k), __dmul_rn(ST(sA, k), rest));
+      t = p.t_end;
+      stop = RT_STOP_T_END;
+      break;
+    }
+    // a-5
+    t = __dadd_rn(t, delta);
+    for (int k = 0; k < M; ++k) ST(sT, k) = __dadd_rn(ST(sT, k), __dmul_rn(ST(sA, k), delta));
+    // a-6
+    for (uint32_t e = s_sp[mu]; e < s_sp[mu + 1]; ++e) {
+      const long long x = ST(sX, s_ss[e]) + (long long)s_sv[e];
+      if (x < 0 || x > net.xmax) status = RT_ERR_OVERFLOW;
+      ST(sX, s_ss[e]) = x;
+    }
+    // a-7
+    const uint32_t c = ST(sN, mu) + 1u;
+    ST(sN, mu) = c;
+    ST(sP, mu) = __dadd_rn(ST(sP, mu), exp_draw(p.seed, traj, (uint32_t)mu, c));
+    fired += 1;
+    if (status != RT_OK) break;
+    if (p.max_firings != 0 && fired == p.max_firings) { stop = RT_STOP_MAX_FIRINGS; break; }
+  }
+
+  if (p.x_out)
+    for (int j = 0; j < N; ++j) p.x_out[it * (u64)N + (u64)j] = ST(sX, j);
+  rt_result res;
+  res.t = t; res.firings = fired; res.stop = stop; res.status = status;
+  p.res[it] = res;
+#undef ST
+}
+
+}  // namespace rt
