@@ -1,0 +1,293 @@
+#!/usr/bin/env python
+"""bench.py -- reaction firings/s of the random-time hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--impl reference]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input: one trajectory of
+the workload's network run for its configured number of firings (cfg4: M=1e6, 1e4 firings) by ONE
+launch of the persistent bundle kernel (a-0 init + every a-1..a-8 of every firing).  `value` is
+timed with CUDA events on the launching stream through rt_run_dev (x0 resident in HBM); `e2e` is
+the host-pointer rt_run (x0 H2D, x_out + result + trace D2H inside the timed region).
+N > 1: the single large-M trajectory does not shard ("replicas only"), so every rank
+runs an independent replica (trajectory id = rank), no collective on the data path.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import rt_workloads as W
+
+METRIC = "reaction firings/sec on 1 B200 at M=10^6 (+ % of HBM roofline per firing)"
+UNIT = "firings/s"
+BYTES_PER_REACTION_FIRING = 32   # read T, P, a; write T
+# Measured once with `ncu --set full` (profiles/): dram bytes per launch of the bundle kernel at
+# the default workload; None until a capture exists for the shipped kernel.
+NCU_TRAFFIC_BYTES = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg3", "cfg4", "cfg5a", "cfg5b"])
+    ap.add_argument("--firings", type=int, default=0, help="firings per step (0 = the config's)")
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink N, M (debug only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--option", action="append", default=[], help="name=value for rt_set_option")
+    return ap.parse_args()
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names)
+                   if any(len(r) >= 6 and r[2 + i].lower() == "active" for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(sm)}
+
+
+def oracle_leg(net, x0, seed, traj, firings):
+    """The oracle as it stands, single thread, timed on the host (wall clock around oracle_run,
+    which includes its own init just as a GPU step includes a-0)."""
+    import oracle
+    t0 = time.perf_counter()
+    o = oracle.run(net, x0, seed, traj, firings, math.inf, 0, want_state=False)
+    dt = time.perf_counter() - t0
+    return o["firings"] / dt, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    net, x0, par = W.make_config(args.workload, scale=args.scale)
+    M = int(net["n_reactions"])
+    # bounded sample: about 2e8 reaction-steps (~2-4 s) per step
+    sample = max(20, min(par["max_firings"], int(2e8 // M)))
+    for _ in range(min(args.warmup, 1)):
+        oracle_leg(net, x0, par["seed"], 0, sample)
+    times, fired = [], 0
+    for _ in range(args.steps):
+        v, dt = oracle_leg(net, x0, par["seed"], 0, sample)
+        times.append(dt)
+        fired += sample
+    value = fired / sum(times)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": args.workload, "n_species": int(net["n_species"]),
+                   "n_reactions": M, "firings_per_step": sample,
+                   "note": "CPU oracle (oracle/rt_oracle.cpp, 1 thread); each step is a bounded "
+                           f"sample: the first {sample} firings of the workload"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": f"first {sample} firings of {args.workload} x {args.steps} steps"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2103_00405_b200 as rt
+
+    rt.lib()                                   # no extension -> ImportError; there is no fallback
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    net, x0, par = W.make_config(args.workload, scale=args.scale)
+    N, M = int(net["n_species"]), int(net["n_reactions"])
+    firings = args.firings or par["max_firings"]
+    n_traj = par["n_traj"]
+    seed = par["seed"]
+    traj0 = rank * n_traj                       # replicas: every rank its own trajectory ids
+    model = rt.Model(net, local)
+    for kv in args.option:
+        k, v = kv.split("=")
+        model.set_option(k, int(v))
+
+    x0_dev = torch.from_numpy(x0).to(dev)
+    x_out_dev = torch.empty(n_traj * N, dtype=torch.int64, device=dev)
+    res_dev = torch.zeros(n_traj * 3, dtype=torch.int64, device=dev)          # rt_result[n_traj]
+    trace_cap = min(firings, par.get("trace", 0)) if n_traj == 1 else 0
+    tmu_dev = torch.empty(max(trace_cap, 1), dtype=torch.int32, device=dev)
+    tt_dev = torch.empty(max(trace_cap, 1), dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)              # > 126 MB L2
+
+    def step_dev():
+        if n_traj == 1:
+            rc = rt.rt_run_dev(model.handle, x0_dev, seed, traj0, firings, math.inf, x_out_dev,
+                               res_dev, tmu_dev, tt_dev, trace_cap)
+        else:
+            rc = rt.rt_ensemble_dev(model.handle, x0_dev, seed, traj0, n_traj, firings, math.inf,
+                                    x_out_dev, res_dev)
+        if rc != rt.RT_OK:
+            raise rt.RtError(rc, "rt_run_dev")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        flush.fill_(1)
+        step_dev()
+    torch.cuda.synchronize()
+    if rt.rt_sync(model.handle) != rt.RT_OK:
+        raise SystemExit("bench.py: device reported an error during warm-up")
+    done = res_dev.cpu().numpy().view(rt.RESULT_DTYPE)
+    assert (done["firings"] == firings).all() and (done["status"] == 0).all(), done
+
+    # ---- timed region: K steps, device-timed; per-step events bracket the kernel launch only
+    # (L2 flush sits between steps, outside the per-step events but inside the barrier bracket).
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    launches0 = model.info("kernel_launches")
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    for a, b in ev:
+        flush.fill_(1)
+        a.record()
+        step_dev()
+        b.record()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    launches = model.info("kernel_launches") - launches0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+    total_s = float(total_ms.item()) * 1e-3
+    units = firings * n_traj * args.steps * world
+    value = units / total_s
+
+    # ---- e2e: the host-pointer C-ABI call a user makes; copies inside the timed region
+    x0_pin = torch.from_numpy(x0.copy()).pin_memory().numpy()
+    e2e_tr = trace_cap
+
+    def step_host():
+        if n_traj == 1:
+            out = model.run(x0_pin, seed, traj0, firings, math.inf, trace_cap=e2e_tr)
+            return out["firings"]
+        out = model.ensemble(x0_pin, seed, traj0, n_traj, firings, math.inf)
+        return int(out["firings"].sum())
+
+    step_host()
+    barrier()
+    t0 = time.perf_counter()
+    got = 0
+    for _ in range(args.steps):
+        got += step_host()
+    torch.cuda.synchronize()
+    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_value = got * world / float(e2e_s.item())
+    h2d = N * 8
+    d2h = n_traj * N * 8 + n_traj * 24 + e2e_tr * 12
+
+    if rank == 0:
+        peak, peak_src = peaks()
+        kernel_s = (sum(step_ms) / len(step_ms)) * 1e-3          # one bundle-kernel launch per step
+        alg_bytes = BYTES_PER_REACTION_FIRING * M * firings * n_traj
+        achieved = alg_bytes / kernel_s / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * total_s / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": args.workload, "n_species": N, "n_reactions": M,
+                       "trajectories_per_step": n_traj, "firings_per_step": firings * n_traj,
+                       "parallelism": "replicas only (one trajectory per GPU)" if n_traj == 1
+                       else "independent trajectories", "l2": "flushed between steps (256 MB fill)",
+                       "bundle_ctas": model.info("bundle_ctas"), "bundles": model.info("bundles"),
+                       "block_threads": model.info("block_threads"),
+                       "us_per_firing": 1e6 * kernel_s / firings},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+                         "kernel": "rt_bundle_kernel", "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": alg_bytes,
+                         "frac_of_8TBs_nominal": achieved / 8000.0},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            sample = max(20, min(firings, int(1e9 // M)))    # ~1e9 reaction-steps: 10-30 s
+            v, dt = oracle_leg(net, x0, seed, traj0, sample)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": f"first {sample} firings of {args.workload} "
+                                              f"(M={M}), {dt:.1f} s, single thread"}
+        print(json.dumps(line))
+    model.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_cuda(a)

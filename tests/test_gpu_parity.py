@@ -1,0 +1,150 @@
+"""GPU parity: the CUDA path (through the C ABI of include/rt.h) against the CPU oracle on the
+same seeded inputs.  Bar (BASELINE.json north_star): fired-reaction sequence and species counts
+bit-exact for the first 1e4 firings, event times within 1e-12 relative."""
+import math
+
+import numpy as np
+import pytest
+
+import rt_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+RTOL_T = 1e-12
+
+
+@pytest.fixture(scope="module")
+def rt():
+    import paper_2103_00405_b200 as rt
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    rt.lib()   # fails loudly if librt_b200.so is missing
+    return rt
+
+
+def _oracle():
+    import oracle
+    return oracle
+
+
+def _check_run(rt, net, x0, seed, traj, max_firings, t_end, trace_cap, options=()):
+    o = _oracle().run(net, x0, seed, traj, max_firings, t_end, trace_cap)
+    with rt.Model(net) as m:
+        for name, val in options:
+            m.set_option(name, val)
+        g = m.run(x0, seed, traj, max_firings, t_end, trace_cap, want_state=True)
+        assert m.info("kernel_launches") >= 1
+    assert g["firings"] == o["firings"]
+    assert g["stop"] == o["stop"]
+    np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["fire_count"], o["fire_count"])
+    np.testing.assert_allclose(g["trace_t"], o["trace_t"], rtol=RTOL_T, atol=0)
+    assert math.isclose(g["t"], o["t"], rel_tol=RTOL_T, abs_tol=0)
+    # internal clocks: sums of a_k*dt, same order on both sides -> agree to ~firings ulp
+    np.testing.assert_allclose(g["T"], o["T"], rtol=1e-10, atol=1e-12)
+    np.testing.assert_allclose(g["P"], o["P"], rtol=1e-12, atol=0)
+    return g, o
+
+
+@pytest.mark.parametrize("refresh_mode", [0, 1])
+@pytest.mark.parametrize("scale,firings", [(0.01, 3000), (0.0517, 2000)])
+def test_cfg3_scaled_trace(rt, scale, firings, refresh_mode):
+    """Random mass-action network at reduced N, M (ragged: M odd / not a tile multiple)."""
+    net, x0, par = W.make_config("cfg3", scale=scale)
+    _check_run(rt, net, x0, par["seed"], 0, firings, math.inf, firings,
+               options=[("refresh_mode", refresh_mode)])
+
+
+@pytest.mark.parametrize("ctas", [1, 2, 7, 0])
+def test_cfg3_bundle_shape_invariance(rt, ctas):
+    """Result must not depend on how many CTAs share the trajectory (determinism contract)."""
+    net, x0, par = W.make_config("cfg3", scale=0.02)
+    _check_run(rt, net, x0, par["seed"], 3, 1500, math.inf, 1500, options=[("bundle_ctas", ctas)])
+
+
+def test_cfg3_full_first_1e4(rt):
+    """BASELINE config 3 at full size: first 1e4 firings bit-exact."""
+    net, x0, par = W.make_config("cfg3")
+    _check_run(rt, net, x0, par["seed"], 0, 10_000, math.inf, 10_000)
+
+
+def test_cfg4_scaled(rt):
+    net, x0, par = W.make_config("cfg4", scale=0.02)
+    _check_run(rt, net, x0, par["seed"], 0, 2000, math.inf, 2000)
+
+
+def test_cfg4_full_prefix(rt):
+    """BASELINE config 4 (M=1e6, the bench workload) in the bench launch shape: the oracle
+    does 300 firings (3e8 reaction-steps) in seconds; compare that prefix bit-exactly."""
+    net, x0, par = W.make_config("cfg4")
+    _check_run(rt, net, x0, par["seed"], 0, 300, math.inf, 300)
+
+
+def test_t_end_stop_and_absorption(rt):
+    net, x0, par = W.make_config("cfg3", scale=0.01)
+    g, o = _check_run(rt, net, x0, 11, 0, 0, 0.002, 4096)
+    assert g["stop"] == rt.RT_STOP_T_END and g["t"] == 0.002
+    # pure death from 5 molecules: absorbed after exactly 5 firings
+    dnet = W.from_reactions(1, [({0: 1}, {}, 0.7)])
+    g, o = _check_run(rt, dnet, np.array([5]), 3, 0, 0, 1e9, 16)
+    assert g["stop"] == rt.RT_STOP_ABSORBED and g["firings"] == 5
+
+
+def test_tiny_networks_on_bundle_path(rt):
+    for builder in (W.birth_death, W.lotka_volterra):
+        net, x0 = builder()
+        _check_run(rt, net, x0, 5, 9, 2000, math.inf, 2000)
+
+
+def test_ensemble_thread_path_matches_oracle(rt):
+    """cfg1 / cfg2 ensembles (one thread per trajectory) against the oracle, row by row."""
+    net, x0, par = W.make_config("cfg1")
+    n = 67
+    o = _oracle().ensemble(net, x0, par["seed"], 5, n, par["max_firings"], 50.0)
+    with rt.Model(net) as m:
+        g = m.ensemble(x0, par["seed"], 5, n, par["max_firings"], 50.0)
+        assert m.info("ensemble_path") == 1
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["firings"], o["firings"])
+    np.testing.assert_array_equal(g["stop"], o["stop"])
+    np.testing.assert_allclose(g["t"], o["t"], rtol=RTOL_T)
+    net, x0, par = W.make_config("cfg2")
+    n = 45
+    o = _oracle().ensemble(net, x0, par["seed"], 0, n, 20_000, 0.5)
+    with rt.Model(net) as m:
+        g = m.ensemble(x0, par["seed"], 0, n, 20_000, 0.5)
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["firings"], o["firings"])
+    np.testing.assert_allclose(g["t"], o["t"], rtol=RTOL_T)
+
+
+def test_ensemble_bundle_path_matches_run_and_oracle(rt):
+    """cfg5b shape (several trajectories of one mid-size network): ensemble row i == rt_run(i)
+    == oracle trajectory i; thread path and bundle path agree on a tiny network."""
+    net, x0, par = W.make_config("cfg5b", scale=0.02)
+    n = 5
+    o = _oracle().ensemble(net, x0, par["seed"], 2, n, 800, math.inf)
+    with rt.Model(net) as m:
+        g = m.ensemble(x0, par["seed"], 2, n, 800, math.inf)
+        assert m.info("ensemble_path") == 2
+        one = m.run(x0, par["seed"], 4, 800)
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_allclose(g["t"], o["t"], rtol=RTOL_T)
+    np.testing.assert_array_equal(one["x"], g["x"][2])
+    net, x0 = W.lotka_volterra()
+    with rt.Model(net) as m:
+        a = m.ensemble(x0, 2, 0, 9, 3000, math.inf)
+        m.set_option("ensemble_path", 2)
+        b = m.ensemble(x0, 2, 0, 9, 3000, math.inf)
+    np.testing.assert_array_equal(a["x"], b["x"])
+    np.testing.assert_array_equal(a["t"], b["t"])
+
+
+def test_prefix_property(rt):
+    net, x0, par = W.make_config("cfg3", scale=0.01)
+    with rt.Model(net) as m:
+        a = m.run(x0, 7, 0, 500, trace_cap=500)
+        b = m.run(x0, 7, 0, 1200, trace_cap=1200)
+    np.testing.assert_array_equal(a["trace_mu"], b["trace_mu"][:500])
+    np.testing.assert_array_equal(a["trace_t"], b["trace_t"][:500])
