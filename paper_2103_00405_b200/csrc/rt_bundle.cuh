@@ -144,9 +144,18 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
   return ctx.win;
 }
 
+#ifdef RT_PHASE_TIMING
+#define PT_DECL long long pt_acc[6] = {0, 0, 0, 0, 0, 0}; long long pt_last = clock64();
+#define PT_MARK(i) { long long now_ = clock64(); pt_acc[i] += now_ - pt_last; pt_last = now_; }
+#else
+#define PT_DECL
+#define PT_MARK(i)
+#endif
+
 template <int BLOCK>
 __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams p) {
   __shared__ BundleCtx<BLOCK> ctx;
+  PT_DECL
   const NetDev &net = p.net;
   const int tid = threadIdx.x;
   const int b = blockIdx.x / p.S, r = blockIdx.x % p.S;
@@ -200,6 +209,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     int mu_prev = -1, stop = 0, status = RT_OK;
 
     for (;;) {
+      PT_MARK(5)
       // ---- A: discrete updates of the previous firing (a-6, a-7, a-8) and refresh flags
       if (mu_prev >= 0) {
         const bool owner = (mu_prev >= k0 && mu_prev < k1);
@@ -232,6 +242,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         __syncthreads();
       }
 
+      PT_MARK(0)
       // ---- B: the streaming pass (a-5 of the previous firing fused with a-2/a-3 of this one)
       Cand best; best.dt = INF; best.k = 0x7fffffff;
       const bool full = (p.refresh_mode != 0);
@@ -269,6 +280,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         }
       }
 
+      PT_MARK(1)
       // ---- C: fix-up -- a-1 for the dependents of the previous firing, from the new X
       if (mu_prev >= 0 && p.refresh_mode == 0) {
         if (tid == 0) wait_xgen(xgen, xg, p.err);
@@ -281,8 +293,10 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         });
       }
 
+      PT_MARK(2)
       // ---- D/E: a-3 argmin over the bundle
       const Cand win = bundle_argmin<BLOCK>(p, ctx, exch, r, gen, best, false);
+      PT_MARK(3)
       if (win.k == -2) return;
 
       // ---- F: a-4 stop tests, identical in every thread of every CTA of the bundle
@@ -332,6 +346,12 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       }
     }
 
+#ifdef RT_PHASE_TIMING
+    if (tid == 0 && (r == 0 || r == p.S - 1 || r == p.S / 2))
+      printf("cta %d: A %.0f B %.0f C %.0f D+E %.0f F %.0f cyc/firing\n", r, (double)pt_acc[0] / fired,
+             (double)pt_acc[1] / fired, (double)pt_acc[2] / fired, (double)pt_acc[3] / fired,
+             (double)pt_acc[5] / fired);
+#endif
     // ---- trajectory done: make X visible bundle-wide, collect the overflow flag, write results
     if (bundle_argmin<BLOCK>(p, ctx, exch, r, gen, none, true).k == -2) return;
     if (ctx.abort_any) status = RT_ERR_OVERFLOW;
