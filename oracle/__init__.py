@@ -79,7 +79,7 @@ def propensities(net, X):
 
 
 def run(net, x0, seed, trajectory=0, max_firings=0, t_end=math.inf, trace_cap=0,
-        want_state=True):
+        want_state=True, check=True):
     """One trajectory.  Returns a dict: x, t, firings, stop, fire_count, T, P, trace_mu, trace_t."""
     args, keep = _net_args(net)
     N, M = int(net["n_species"]), int(net["n_reactions"])
@@ -99,10 +99,10 @@ def run(net, x0, seed, trajectory=0, max_firings=0, t_end=math.inf, trace_cap=0,
                           C.byref(t), C.byref(firings), C.byref(stop), _p(fc, C.c_uint64),
                           _p(T, C.c_double), _p(P, C.c_double), _p(tmu, C.c_int32),
                           _p(tt, C.c_double), C.c_uint64(trace_cap))
-    if rc != 0:
+    if rc != 0 and check:
         raise RuntimeError(f"oracle_run failed with code {rc}")
     nrec = min(int(firings.value), trace_cap)
-    return dict(x=x, t=t.value, firings=int(firings.value), stop=int(stop.value),
+    return dict(x=x, t=t.value, firings=int(firings.value), stop=int(stop.value), code=rc,
                 fire_count=fc, T=T, P=P,
                 trace_mu=None if tmu is None else tmu[:nrec],
                 trace_t=None if tt is None else tt[:nrec])

@@ -20,9 +20,12 @@ using rt::u64;
 
 namespace {
 
-constexpr int kBlock = 1024;          // threads per CTA of the bundle kernel
+constexpr int kBlock = 1024;          // threads per CTA of the bundle kernel (31 stream warps + 1 walker)
 constexpr int kThreadKernelMaxM = 64; // one-thread-per-trajectory path: M, N at most this
 constexpr int kMinPairsPerCta = 256;  // do not spread a trajectory thinner than this
+constexpr int kBigDeg = 64;           // species read by more reactions than this get a block-offset table
+constexpr int kTargetBlocks = 256;    // ... with about this many reaction blocks
+constexpr size_t kSmemStateBytes = 208 * 1024;   // dynamic shared memory the (T,P,a) state may take
 
 #define CU_TRY(expr)                                                         \
   do {                                                                       \
@@ -60,16 +63,17 @@ struct rt_model {
   int max_sigma = 1;
   // device copies of the network
   DevBuf d_react_ptr, d_react_species, d_react_sigma, d_stoich_ptr, d_stoich_species, d_stoich_v,
-      d_rate, d_dep_ptr, d_dep_rxn;
+      d_rate, d_srow_j, d_srow_v, d_sp_rec, d_sp_big, d_big_off, d_dep;
   // per-bundle state
-  DevBuf d_T, d_P, d_a, d_n, d_X, d_exch, d_xgen, d_err;
+  DevBuf d_T, d_P, d_a, d_n, d_X, d_exch, d_err;
   // staging for the host-pointer API
   DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t;
   // options
-  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0;
+  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0;
   // info
   int64_t kernel_launches = 0;
-  int last_S = 0, last_B = 0, last_path = 0;
+  int last_S = 0, last_B = 0, last_path = 0, last_state_smem = 0;
+  size_t n_big = 0;
 };
 
 namespace {
@@ -130,26 +134,34 @@ int upload(DevBuf &buf, const std::vector<T> &host) {
   return RT_OK;
 }
 
-// How one launch is shaped: B bundles of S CTAs.
-struct Plan { int S, B; int pairs_per_cta; };
+// How one launch is shaped: B bundles of S CTAs; smem = the (T,P,a) state lives in shared memory.
+struct Plan { int S, B; int pairs_per_cta; bool smem; };
+
+size_t smem_state_bytes(int pairs_per_cta) { return (size_t)pairs_per_cta * 2 * 3 * sizeof(double); }
 
 Plan plan_bundles(const rt_model *m, u64 n_traj) {
   const int pairs_total = m->net.M_pad / 2;
   const int sms = m->num_sms;
+  // fewest CTAs whose share of the state still fits in shared memory
+  const int pairs_fit = (int)(kSmemStateBytes / (2 * 3 * sizeof(double)));
+  const int s_fit = (pairs_total + pairs_fit - 1) / pairs_fit;
+  const int s_thin = std::max(1, (pairs_total + kMinPairsPerCta - 1) / kMinPairsPerCta);
   int S;
   if (m->opt_bundle_ctas > 0) {
     S = std::min(m->opt_bundle_ctas, sms);
   } else if (n_traj <= 1) {
-    S = sms;                                            // one trajectory: the whole chip
+    S = std::min(sms, s_thin);                          // one trajectory: the whole chip
   } else {
-    S = (int)std::max<u64>(1, (u64)sms / n_traj);       // many: as many bundles as fit
+    S = (int)std::max<u64>(1, (u64)sms / n_traj);       // many: as many bundles as fit ...
+    if (m->opt_state_mode != 1 && S < s_fit && s_fit <= sms) S = s_fit;   // ... with on-chip state
+    S = std::min(S, s_thin);
   }
-  S = std::min(S, std::max(1, (pairs_total + kMinPairsPerCta - 1) / kMinPairsPerCta));
   S = std::max(S, 1);
   Plan pl;
   pl.S = S;
   pl.B = (int)std::min<u64>(std::max<u64>(n_traj, 1), (u64)(sms / S));
   pl.pairs_per_cta = (pairs_total + S - 1) / S;
+  pl.smem = m->opt_state_mode != 1 && smem_state_bytes(pl.pairs_per_cta) <= kSmemStateBytes;
   return pl;
 }
 
@@ -160,9 +172,8 @@ int ensure_state(rt_model *m, const Plan &pl) {
   if ((rc = m->d_P.ensure(B * Mp * 8)) != RT_OK) return rc;
   if ((rc = m->d_a.ensure(B * Mp * 8)) != RT_OK) return rc;
   if ((rc = m->d_n.ensure(B * Mp * 4)) != RT_OK) return rc;
-  if ((rc = m->d_X.ensure(B * N * 8)) != RT_OK) return rc;
+  if ((rc = m->d_X.ensure(B * (size_t)pl.S * N * 8)) != RT_OK) return rc;   // one replica per CTA
   if ((rc = m->d_exch.ensure(B * 2 * (size_t)pl.S * 2 * 8)) != RT_OK) return rc;
-  if ((rc = m->d_xgen.ensure(B * 32 * 4)) != RT_OK) return rc;
   if ((rc = m->d_err.ensure(16)) != RT_OK) return rc;
   return RT_OK;
 }
@@ -174,12 +185,11 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   int rc = ensure_state(m, pl);
   if (rc != RT_OK) return rc;
   CU_TRY(cudaMemsetAsync(m->d_exch.p, 0, (size_t)pl.B * 2 * pl.S * 2 * 8, st));
-  CU_TRY(cudaMemsetAsync(m->d_xgen.p, 0, (size_t)pl.B * 32 * 4, st));
   rt::BundleParams p{};
   p.net = m->net;
   p.T = (double *)m->d_T.p; p.P = (double *)m->d_P.p; p.a = (double *)m->d_a.p;
   p.n = (uint32_t *)m->d_n.p; p.X = (long long *)m->d_X.p;
-  p.exch = (u64 *)m->d_exch.p; p.xgen = (uint32_t *)m->d_xgen.p;
+  p.exch = (u64 *)m->d_exch.p;
   p.S = pl.S; p.B = pl.B; p.pairs_per_cta = pl.pairs_per_cta;
   p.x0 = x0_dev; p.seed = seed; p.traj_first = traj_first; p.n_traj = n_traj;
   p.max_firings = max_firings; p.t_end = t_end;
@@ -190,10 +200,18 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.err = (int *)m->d_err.p;
   void *args[] = {&p};
   // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
-  CU_TRY(cudaLaunchCooperativeKernel((const void *)rt::rt_bundle_kernel<kBlock>, dim3(pl.S * pl.B),
-                                     dim3(kBlock), args, 0, st));
+  if (pl.smem) {
+    const size_t dyn = smem_state_bytes(pl.pairs_per_cta);
+    CU_TRY(cudaFuncSetAttribute(rt::rt_bundle_kernel<kBlock, true>,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+    CU_TRY(cudaLaunchCooperativeKernel((const void *)rt::rt_bundle_kernel<kBlock, true>,
+                                       dim3(pl.S * pl.B), dim3(kBlock), args, dyn, st));
+  } else {
+    CU_TRY(cudaLaunchCooperativeKernel((const void *)rt::rt_bundle_kernel<kBlock, false>,
+                                       dim3(pl.S * pl.B), dim3(kBlock), args, 0, st));
+  }
   m->kernel_launches += 1;
-  m->last_S = pl.S; m->last_B = pl.B; m->last_path = 2;
+  m->last_S = pl.S; m->last_B = pl.B; m->last_path = 2; m->last_state_smem = pl.smem ? 1 : 0;
   return RT_OK;
 }
 
@@ -285,16 +303,57 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
       rg(net->react_sigma, net->react_sigma + nr), ss(net->stoich_species, net->stoich_species + nv),
       sv(net->stoich_v, net->stoich_v + nv);
   std::vector<double> rate(net->rate, net->rate + M);
-  // dependency lists: species j -> reactions with j as a reactant, ascending reaction index
-  // (counting sort over the reactant CSR, which is already ordered by reaction).
+  // ---- dependency graph, two-hop: stoich row of mu -> species -> reactions that
+  // have the species as a reactant.  Entries of one species ascend in k (counting sort over the
+  // reactant CSR, which is ordered by reaction) and carry what a refresh needs.
   std::vector<uint32_t> dp((size_t)N + 1, 0u);
   for (size_t e = 0; e < nr; ++e) dp[(size_t)rs[e] + 1] += 1u;
   for (int32_t j = 0; j < N; ++j) dp[j + 1] += dp[j];
-  std::vector<int32_t> dr(nr);
+  std::vector<int32_t> dep(4 * std::max<size_t>(nr, 1), 0);
   {
     std::vector<uint32_t> cursor(dp.begin(), dp.end() - 1);
-    for (int32_t k = 0; k < M; ++k)
-      for (uint32_t e = rp[k]; e < rp[k + 1]; ++e) dr[cursor[rs[e]]++] = k;
+    for (int32_t k = 0; k < M; ++k) {
+      const uint32_t rb = rp[k], re = rp[k + 1];
+      const int32_t j1 = rs[rb < re ? rb : 0], s1 = rg[rb < re ? rb : 0];
+      const int32_t j2 = (re - rb >= 2) ? rs[rb + 1] : -1, s2 = (re - rb >= 2) ? rg[rb + 1] : 0;
+      const int32_t flags = s1 | (s2 << 8) | ((re - rb > 2) ? 0x10000 : 0);
+      for (uint32_t e = rb; e < re; ++e) {
+        const size_t at = 4 * (size_t)cursor[rs[e]]++;
+        dep[at] = k; dep[at + 1] = j1; dep[at + 2] = j2; dep[at + 3] = flags;
+      }
+    }
+  }
+  std::vector<uint32_t> sp_rec(2 * (size_t)N);
+  std::vector<int32_t> sp_big((size_t)N, -1);
+  int blk_shift = 0;
+  while (((int64_t)M >> blk_shift) > kTargetBlocks) ++blk_shift;
+  const int n_blk = (int)(((int64_t)M + (1ll << blk_shift) - 1) >> blk_shift) + 1;   // + the odd pad
+  size_t n_big = 0;
+  for (int32_t j = 0; j < N; ++j) {
+    sp_rec[2 * (size_t)j] = dp[j];
+    sp_rec[2 * (size_t)j + 1] = dp[j + 1];
+    if (dp[j + 1] - dp[j] > (uint32_t)kBigDeg) sp_big[j] = (int32_t)n_big++;
+  }
+  std::vector<uint32_t> big_off(std::max<size_t>(n_big * (size_t)(n_blk + 1), 1), 0u);
+  for (int32_t j = 0; j < N; ++j) {
+    if (sp_big[j] < 0) continue;
+    uint32_t *off = big_off.data() + (size_t)sp_big[j] * (size_t)(n_blk + 1);
+    uint32_t i = dp[j];
+    for (int bq = 0; bq <= n_blk; ++bq) {      // off[bq] = first entry with k >= bq << blk_shift
+      const int64_t kmin = (int64_t)bq << blk_shift;
+      while (i < dp[j + 1] && (int64_t)dep[4 * (size_t)i] < kmin) ++i;
+      off[bq] = i;
+    }
+  }
+  // ELL copy of the stoich rows (up to 4 changed species per reaction)
+  std::vector<int32_t> srow_j(4 * (size_t)M, -1), srow_v(4 * (size_t)M, 0);
+  for (int32_t k = 0; k < M; ++k) {
+    const uint32_t sb = sp[k], se = sp[k + 1];
+    if (se - sb > 4) { srow_j[4 * (size_t)k] = -2; continue; }
+    for (uint32_t e = sb; e < se; ++e) {
+      srow_j[4 * (size_t)k + (e - sb)] = ss[e];
+      srow_v[4 * (size_t)k + (e - sb)] = sv[e];
+    }
   }
   rc = RT_OK;
   if (rc == RT_OK) rc = upload(m->d_react_ptr, rp);
@@ -304,8 +363,12 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
   if (rc == RT_OK) rc = upload(m->d_stoich_species, ss);
   if (rc == RT_OK) rc = upload(m->d_stoich_v, sv);
   if (rc == RT_OK) rc = upload(m->d_rate, rate);
-  if (rc == RT_OK) rc = upload(m->d_dep_ptr, dp);
-  if (rc == RT_OK) rc = upload(m->d_dep_rxn, dr);
+  if (rc == RT_OK) rc = upload(m->d_srow_j, srow_j);
+  if (rc == RT_OK) rc = upload(m->d_srow_v, srow_v);
+  if (rc == RT_OK) rc = upload(m->d_sp_rec, sp_rec);
+  if (rc == RT_OK) rc = upload(m->d_sp_big, sp_big);
+  if (rc == RT_OK) rc = upload(m->d_big_off, big_off);
+  if (rc == RT_OK) rc = upload(m->d_dep, dep);
   if (rc == RT_OK) rc = m->d_err.ensure(16);
   if (rc == RT_OK && cudaMemset(m->d_err.p, 0, 16) != cudaSuccess) rc = RT_ERR_CUDA;
   if (rc != RT_OK) { rt_destroy(m); return rc; }
@@ -320,8 +383,14 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
   d.stoich_species = (const int32_t *)m->d_stoich_species.p;
   d.stoich_v = (const int32_t *)m->d_stoich_v.p;
   d.rate = (const double *)m->d_rate.p;
-  d.dep_ptr = (const uint32_t *)m->d_dep_ptr.p;
-  d.dep_rxn = (const int32_t *)m->d_dep_rxn.p;
+  d.srow_j = (const int32_t *)m->d_srow_j.p;
+  d.srow_v = (const int32_t *)m->d_srow_v.p;
+  d.sp_rec = (const uint32_t *)m->d_sp_rec.p;
+  d.sp_big = (const int32_t *)m->d_sp_big.p;
+  d.big_off = (const uint32_t *)m->d_big_off.p;
+  d.dep = (const int32_t *)m->d_dep.p;
+  d.n_blk = n_blk; d.blk_shift = blk_shift; d.big_deg = kBigDeg;
+  m->n_big = n_big;
   d.xmax = max_sigma <= 2 ? ((1ll << 31) - 1) : ((1ll << 21) - 1);
   *out = m;
   return RT_OK;
@@ -447,6 +516,9 @@ int rt_set_option(rt_model *m, const char *name, int64_t value) {
   } else if (!strcmp(name, "ensemble_path")) {
     if (value < 0 || value > 2) return RT_ERR_BAD_ARG;
     m->opt_ensemble_path = (int)value;
+  } else if (!strcmp(name, "state_mode")) {
+    if (value < 0 || value > 1) return RT_ERR_BAD_ARG;
+    m->opt_state_mode = (int)value;
   } else {
     return RT_ERR_BAD_ARG;
   }
@@ -463,6 +535,8 @@ int rt_get_info(const rt_model *m, const char *name, int64_t *value) {
   else if (!strcmp(name, "num_sms")) *value = m->num_sms;
   else if (!strcmp(name, "dep_entries")) *value = m->nnz_r;
   else if (!strcmp(name, "max_sigma")) *value = m->max_sigma;
+  else if (!strcmp(name, "state_in_smem")) *value = m->last_state_smem;
+  else if (!strcmp(name, "hub_species")) *value = (int64_t)m->n_big;
   else return RT_ERR_BAD_ARG;
   return RT_OK;
 }
@@ -471,8 +545,9 @@ void rt_destroy(rt_model *m) {
   if (!m) return;
   cudaSetDevice(m->device);
   DevBuf *bufs[] = {&m->d_react_ptr, &m->d_react_species, &m->d_react_sigma, &m->d_stoich_ptr,
-                    &m->d_stoich_species, &m->d_stoich_v, &m->d_rate, &m->d_dep_ptr, &m->d_dep_rxn,
-                    &m->d_T, &m->d_P, &m->d_a, &m->d_n, &m->d_X, &m->d_exch, &m->d_xgen, &m->d_err,
+                    &m->d_stoich_species, &m->d_stoich_v, &m->d_rate, &m->d_srow_j, &m->d_srow_v,
+                    &m->d_sp_rec, &m->d_sp_big, &m->d_big_off, &m->d_dep,
+                    &m->d_T, &m->d_P, &m->d_a, &m->d_n, &m->d_X, &m->d_exch, &m->d_err,
                     &m->d_x0, &m->d_xout, &m->d_res, &m->d_trace_mu, &m->d_trace_t};
   for (DevBuf *b : bufs) b->release();
   delete m;

@@ -23,8 +23,16 @@ struct NetDev {
   const int32_t *stoich_species; // [nnz_v]
   const int32_t *stoich_v;       // [nnz_v]
   const double *rate;            // [M]
-  const uint32_t *dep_ptr;       // [N+1]  species j -> reactions that have j as a reactant
-  const int32_t *dep_rxn;        // [nnz_r] sorted by reaction index within a species
+  // Dependency graph, stored two-hop and dense so that a walk is three
+  // dependent loads: stoich row of mu -> species record -> dependency entries.
+  const int32_t *srow_j;         // [M][4] changed species of reaction k (ELL copy of its stoich row;
+  const int32_t *srow_v;         // [M][4]  v = 0: unused slot; srow_j[k][0] = -2: row has > 4 entries)
+  const uint32_t *sp_rec;        // [N][2] (lo, hi): entries of species j in dep[]
+  const int32_t *sp_big;         // [N]    row of big_off for hub species (degree > big_deg), else -1
+  const uint32_t *big_off;       // [n_big][n_blk+1] hub species: first entry with k >= b << blk_shift
+  const int32_t *dep;            // [nnz_r][4] (k, j1, j2 or -1, sigma1 | sigma2 << 8 | general << 16),
+                                 //        sorted by k within a species; (j1, j2) = first two reactants of k
+  int32_t n_blk, blk_shift, big_deg;
   long long xmax;                // count bound (2^31-1, or 2^21-1 if some sigma = 3)
 };
 
@@ -69,12 +77,12 @@ __device__ __forceinline__ long long binom(long long x, int sigma) {
 }
 
 // a_k = c_k * prod_j C(X_j, sigma_jk): one rounded multiply per reactant, CSR order.
-// X is read with ld.global.cg (L2): another CTA may have written it since this SM's L1 saw it.
+// X is the calling CTA's private replica (or shared memory), so plain loads are coherent.
 __device__ __forceinline__ double propensity(const NetDev &net, const long long *X, int k) {
   double a = __ldg(net.rate + k);
   const uint32_t e1 = __ldg(net.react_ptr + k + 1);
   for (uint32_t e = __ldg(net.react_ptr + k); e < e1; ++e) {
-    const long long x = __ldcg(X + __ldg(net.react_species + e));
+    const long long x = X[__ldg(net.react_species + e)];
     a = __dmul_rn(a, __ll2double_rn(binom(x, __ldg(net.react_sigma + e))));
   }
   return a;
@@ -98,8 +106,7 @@ __device__ __forceinline__ Cand warp_lexmin(Cand c) {
   return c;
 }
 
-// Waiting time of one channel (Eq.24 with constant a_k; readings G4, G7): a <= 0 (which
-// includes "flagged for refresh", stored as -|a|, and a = -0.0) gives +inf.
+// Waiting time of one channel (Eq.24 with constant a_k; readings G4, G7): a = 0 gives +inf.
 __device__ __forceinline__ double waiting_time(double P, double T, double a) {
   if (!(a > 0.0)) return __longlong_as_double(0x7ff0000000000000ll);
   double r = __dsub_rn(P, T);

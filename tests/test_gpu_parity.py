@@ -63,6 +63,59 @@ def test_cfg3_bundle_shape_invariance(rt, ctas):
     _check_run(rt, net, x0, par["seed"], 3, 1500, math.inf, 1500, options=[("bundle_ctas", ctas)])
 
 
+@pytest.mark.parametrize("state_mode", [0, 1])
+@pytest.mark.parametrize("ctas", [1, 3, 0])
+def test_state_in_shared_vs_global_memory(rt, state_mode, ctas):
+    """The (T,P,a) store lives in shared memory when a CTA's share fits, else in global memory
+    (the HBM-streaming regime of cfg5a); both must give the oracle's path."""
+    net, x0, par = W.make_config("cfg3", scale=0.03)
+    _check_run(rt, net, x0, par["seed"], 1, 1200, math.inf, 1200,
+               options=[("state_mode", state_mode), ("bundle_ctas", ctas)])
+
+
+def _hub_network(n_species=40, n_reactions=5000, seed=3):
+    """Every reaction reads hub species 0 (degree 5000 >> the hub threshold and, on one CTA,
+    more refreshes per firing than one staging round holds); some rows have 3 reactants
+    (general propensity path) and some change 6 species (CSR stoich path)."""
+    rng = np.random.default_rng(seed)
+    reactions = []
+    for k in range(n_reactions):
+        others = rng.choice(np.arange(1, n_species), size=6, replace=False)
+        reactants = {0: 1}
+        kind = k % 5
+        if kind >= 1:
+            reactants[int(others[0])] = 1 + (k % 2)
+        if kind == 4:
+            reactants[int(others[1])] = 1
+        products = {0: 1, int(others[2]): 1}
+        if kind == 3:
+            products.update({int(others[3]): 1, int(others[4]): 2, int(others[5]): 1})
+        reactions.append((reactants, products, float(10.0 ** rng.uniform(-4, -2))))
+    return W.from_reactions(n_species, reactions), rng.integers(20, 60, size=n_species).astype(np.int64)
+
+
+@pytest.mark.parametrize("ctas,state_mode", [(1, 0), (1, 1), (5, 0), (0, 0)])
+def test_hub_species_general_rows_and_staging_overflow(rt, ctas, state_mode):
+    net, x0 = _hub_network()
+    for refresh_mode in (0, 1):
+        _check_run(rt, net, x0, 21, 0, 600, math.inf, 600,
+                   options=[("bundle_ctas", ctas), ("state_mode", state_mode),
+                            ("refresh_mode", refresh_mode)])
+
+
+def test_count_overflow_is_reported(rt):
+    """0 -> X from the count bound: the first firing leaves [0, 2^31-1] -> RT_ERR_OVERFLOW."""
+    net = W.from_reactions(2, [({}, {0: 1}, 1.0), ({1: 1}, {}, 1.0)])
+    x0 = np.array([2**31 - 1, 3], dtype=np.int64)
+    o = _oracle().run(net, x0, 5, 0, 100, math.inf, 100, check=False)
+    with rt.Model(net) as m:
+        g = m.run(x0, 5, 0, 100, math.inf, 100, check=False)
+    assert g["code"] == rt.RT_ERR_OVERFLOW and g["status"] == rt.RT_ERR_OVERFLOW
+    assert g["firings"] == o["firings"]
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
+
+
 def test_cfg3_full_first_1e4(rt):
     """BASELINE config 3 at full size: first 1e4 firings bit-exact."""
     net, x0, par = W.make_config("cfg3")
