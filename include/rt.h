@@ -95,8 +95,9 @@ int rt_create(const rt_network *net, int device, rt_model **out);
  *   next internal firing times -- each may be NULL.
  *   trace_mu/trace_t [trace_cap]: the fired reaction and the time of each of the first trace_cap
  *   firings (either may be NULL; trace_cap may be 0).
- * Returns RT_ERR_OVERFLOW (also in res->status) if a count left the bound; outputs then hold the
- * state at the offending firing. */
+ * Returns RT_ERR_OVERFLOW (also in res->status) if a firing would take a count out of the bound
+ * (or after 2^33-2 firings of one trajectory): that firing is counted in res->firings and in the
+ * trace, its internal-time increment and redraw are applied, its change of X is not. */
 int rt_run(rt_model *m, const int64_t *x0, uint64_t seed, uint64_t trajectory,
            uint64_t max_firings, double t_end,
            int64_t *x_out, rt_result *res,

@@ -18,9 +18,12 @@
 
 using rt::u64;
 
+#ifndef RT_BLOCK
+#define RT_BLOCK 512
+#endif
 namespace {
 
-constexpr int kBlock = 1024;          // threads per CTA of the bundle kernel (31 stream warps + 1 walker)
+constexpr int kBlock = RT_BLOCK;          // threads per CTA of the bundle kernel (stream warps + 1 walker warp)
 constexpr int kThreadKernelMaxM = 64; // one-thread-per-trajectory path: M, N at most this
 constexpr int kMinPairsPerCta = 256;  // do not spread a trajectory thinner than this
 constexpr int kBigDeg = 64;           // species read by more reactions than this get a block-offset table
@@ -63,13 +66,13 @@ struct rt_model {
   int max_sigma = 1;
   // device copies of the network
   DevBuf d_react_ptr, d_react_species, d_react_sigma, d_stoich_ptr, d_stoich_species, d_stoich_v,
-      d_rate, d_srow_j, d_srow_v, d_sp_rec, d_sp_big, d_big_off, d_dep;
+      d_rate, d_srow, d_sp_rec, d_sp_big, d_big_off, d_dep;
   // per-bundle state
   DevBuf d_T, d_P, d_a, d_n, d_X, d_exch, d_err;
   // staging for the host-pointer API
   DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t;
   // options
-  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0;
+  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0;
   // info
   int64_t kernel_launches = 0;
   int last_S = 0, last_B = 0, last_path = 0, last_state_smem = 0;
@@ -135,7 +138,7 @@ int upload(DevBuf &buf, const std::vector<T> &host) {
 }
 
 // How one launch is shaped: B bundles of S CTAs; smem = the (T,P,a) state lives in shared memory.
-struct Plan { int S, B; int pairs_per_cta; bool smem; };
+struct Plan { int S, B, G; int pairs_per_cta; bool smem; };
 
 size_t smem_state_bytes(int pairs_per_cta) { return (size_t)pairs_per_cta * 2 * 3 * sizeof(double); }
 
@@ -156,11 +159,13 @@ Plan plan_bundles(const rt_model *m, u64 n_traj) {
     if (m->opt_state_mode != 1 && S < s_fit && s_fit <= sms) S = s_fit;   // ... with on-chip state
     S = std::min(S, s_thin);
   }
-  S = std::max(S, 1);
+  S = std::max(std::min(S, rt::kMaxBundleCtas), 1);
   Plan pl;
   pl.S = S;
   pl.B = (int)std::min<u64>(std::max<u64>(n_traj, 1), (u64)(sms / S));
   pl.pairs_per_cta = (pairs_total + S - 1) / S;
+  pl.G = std::min(S, m->opt_x_replicas > 0 ? m->opt_x_replicas : 1);      // X replicas: spread the per-firing reads/atomics of hot species
+  while (pl.G > 1 && (size_t)pl.B * pl.G * (size_t)m->net.N * 8 > ((size_t)64 << 20)) pl.G /= 2;
   pl.smem = m->opt_state_mode != 1 && smem_state_bytes(pl.pairs_per_cta) <= kSmemStateBytes;
   return pl;
 }
@@ -172,8 +177,8 @@ int ensure_state(rt_model *m, const Plan &pl) {
   if ((rc = m->d_P.ensure(B * Mp * 8)) != RT_OK) return rc;
   if ((rc = m->d_a.ensure(B * Mp * 8)) != RT_OK) return rc;
   if ((rc = m->d_n.ensure(B * Mp * 4)) != RT_OK) return rc;
-  if ((rc = m->d_X.ensure(B * (size_t)pl.S * N * 8)) != RT_OK) return rc;   // one replica per CTA
-  if ((rc = m->d_exch.ensure(B * 2 * (size_t)pl.S * 2 * 8)) != RT_OK) return rc;
+  if ((rc = m->d_X.ensure(B * (size_t)pl.G * N * 8)) != RT_OK) return rc;
+  if ((rc = m->d_exch.ensure(B * 2 * (size_t)pl.S * rt::kSlotStride * 8)) != RT_OK) return rc;
   if ((rc = m->d_err.ensure(16)) != RT_OK) return rc;
   return RT_OK;
 }
@@ -184,13 +189,13 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   const Plan pl = plan_bundles(m, n_traj);
   int rc = ensure_state(m, pl);
   if (rc != RT_OK) return rc;
-  CU_TRY(cudaMemsetAsync(m->d_exch.p, 0, (size_t)pl.B * 2 * pl.S * 2 * 8, st));
+  CU_TRY(cudaMemsetAsync(m->d_exch.p, 0, (size_t)pl.B * 2 * pl.S * rt::kSlotStride * 8, st));
   rt::BundleParams p{};
   p.net = m->net;
   p.T = (double *)m->d_T.p; p.P = (double *)m->d_P.p; p.a = (double *)m->d_a.p;
-  p.n = (uint32_t *)m->d_n.p; p.X = (long long *)m->d_X.p;
+  p.n = (uint32_t *)m->d_n.p; p.X = (u64 *)m->d_X.p;
   p.exch = (u64 *)m->d_exch.p;
-  p.S = pl.S; p.B = pl.B; p.pairs_per_cta = pl.pairs_per_cta;
+  p.S = pl.S; p.B = pl.B; p.G = pl.G; p.pairs_per_cta = pl.pairs_per_cta;
   p.x0 = x0_dev; p.seed = seed; p.traj_first = traj_first; p.n_traj = n_traj;
   p.max_firings = max_firings; p.t_end = t_end;
   p.x_out = x_out_dev; p.res = res_dev;
@@ -309,7 +314,7 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
   std::vector<uint32_t> dp((size_t)N + 1, 0u);
   for (size_t e = 0; e < nr; ++e) dp[(size_t)rs[e] + 1] += 1u;
   for (int32_t j = 0; j < N; ++j) dp[j + 1] += dp[j];
-  std::vector<int32_t> dep(4 * std::max<size_t>(nr, 1), 0);
+  std::vector<int32_t> dep(8 * std::max<size_t>(nr, 1), 0);      // 32-byte entries
   {
     std::vector<uint32_t> cursor(dp.begin(), dp.end() - 1);
     for (int32_t k = 0; k < M; ++k) {
@@ -318,8 +323,9 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
       const int32_t j2 = (re - rb >= 2) ? rs[rb + 1] : -1, s2 = (re - rb >= 2) ? rg[rb + 1] : 0;
       const int32_t flags = s1 | (s2 << 8) | ((re - rb > 2) ? 0x10000 : 0);
       for (uint32_t e = rb; e < re; ++e) {
-        const size_t at = 4 * (size_t)cursor[rs[e]]++;
+        const size_t at = 8 * (size_t)cursor[rs[e]]++;
         dep[at] = k; dep[at + 1] = j1; dep[at + 2] = j2; dep[at + 3] = flags;
+        memcpy(&dep[at + 4], &rate[k], sizeof(double));
       }
     }
   }
@@ -341,18 +347,23 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
     uint32_t i = dp[j];
     for (int bq = 0; bq <= n_blk; ++bq) {      // off[bq] = first entry with k >= bq << blk_shift
       const int64_t kmin = (int64_t)bq << blk_shift;
-      while (i < dp[j + 1] && (int64_t)dep[4 * (size_t)i] < kmin) ++i;
+      while (i < dp[j + 1] && (int64_t)dep[8 * (size_t)i] < kmin) ++i;
       off[bq] = i;
     }
   }
-  // ELL copy of the stoich rows (up to 4 changed species per reaction)
-  std::vector<int32_t> srow_j(4 * (size_t)M, -1), srow_v(4 * (size_t)M, 0);
+  // ELL copy of the stoich rows: up to 4 x (j, v, lo, hi), 64 bytes per reaction
+  std::vector<int32_t> srow(16 * (size_t)M);
   for (int32_t k = 0; k < M; ++k) {
+    int32_t *row = srow.data() + 16 * (size_t)k;
+    for (int e = 0; e < 4; ++e) { row[4 * e] = -1; row[4 * e + 1] = 0; row[4 * e + 2] = 0; row[4 * e + 3] = 0; }
     const uint32_t sb = sp[k], se = sp[k + 1];
-    if (se - sb > 4) { srow_j[4 * (size_t)k] = -2; continue; }
+    if (se - sb > 4) { row[0] = -2; continue; }
     for (uint32_t e = sb; e < se; ++e) {
-      srow_j[4 * (size_t)k + (e - sb)] = ss[e];
-      srow_v[4 * (size_t)k + (e - sb)] = sv[e];
+      const int32_t j = ss[e];
+      int32_t *q = row + 4 * (e - sb);
+      q[0] = j; q[1] = sv[e];
+      if (sp_big[j] >= 0) { q[2] = sp_big[j]; q[3] = (int32_t)0xffffffffu; }
+      else { q[2] = (int32_t)dp[j]; q[3] = (int32_t)dp[j + 1]; }
     }
   }
   rc = RT_OK;
@@ -363,8 +374,7 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
   if (rc == RT_OK) rc = upload(m->d_stoich_species, ss);
   if (rc == RT_OK) rc = upload(m->d_stoich_v, sv);
   if (rc == RT_OK) rc = upload(m->d_rate, rate);
-  if (rc == RT_OK) rc = upload(m->d_srow_j, srow_j);
-  if (rc == RT_OK) rc = upload(m->d_srow_v, srow_v);
+  if (rc == RT_OK) rc = upload(m->d_srow, srow);
   if (rc == RT_OK) rc = upload(m->d_sp_rec, sp_rec);
   if (rc == RT_OK) rc = upload(m->d_sp_big, sp_big);
   if (rc == RT_OK) rc = upload(m->d_big_off, big_off);
@@ -383,8 +393,7 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
   d.stoich_species = (const int32_t *)m->d_stoich_species.p;
   d.stoich_v = (const int32_t *)m->d_stoich_v.p;
   d.rate = (const double *)m->d_rate.p;
-  d.srow_j = (const int32_t *)m->d_srow_j.p;
-  d.srow_v = (const int32_t *)m->d_srow_v.p;
+  d.srow = (const int32_t *)m->d_srow.p;
   d.sp_rec = (const uint32_t *)m->d_sp_rec.p;
   d.sp_big = (const int32_t *)m->d_sp_big.p;
   d.big_off = (const uint32_t *)m->d_big_off.p;
@@ -516,6 +525,9 @@ int rt_set_option(rt_model *m, const char *name, int64_t value) {
   } else if (!strcmp(name, "ensemble_path")) {
     if (value < 0 || value > 2) return RT_ERR_BAD_ARG;
     m->opt_ensemble_path = (int)value;
+  } else if (!strcmp(name, "x_replicas")) {
+    if (value < 0 || value > 64) return RT_ERR_BAD_ARG;
+    m->opt_x_replicas = (int)value;
   } else if (!strcmp(name, "state_mode")) {
     if (value < 0 || value > 1) return RT_ERR_BAD_ARG;
     m->opt_state_mode = (int)value;
@@ -545,13 +557,19 @@ void rt_destroy(rt_model *m) {
   if (!m) return;
   cudaSetDevice(m->device);
   DevBuf *bufs[] = {&m->d_react_ptr, &m->d_react_species, &m->d_react_sigma, &m->d_stoich_ptr,
-                    &m->d_stoich_species, &m->d_stoich_v, &m->d_rate, &m->d_srow_j, &m->d_srow_v,
+                    &m->d_stoich_species, &m->d_stoich_v, &m->d_rate, &m->d_srow,
                     &m->d_sp_rec, &m->d_sp_big, &m->d_big_off, &m->d_dep,
                     &m->d_T, &m->d_P, &m->d_a, &m->d_n, &m->d_X, &m->d_exch, &m->d_err,
                     &m->d_x0, &m->d_xout, &m->d_res, &m->d_trace_mu, &m->d_trace_t};
   for (DevBuf *b : bufs) b->release();
   delete m;
 }
+
+#ifdef RT_PHASE_TIMING
+int rt_debug_dump(unsigned long long *out) {
+  return cudaMemcpyFromSymbol(out, rt::g_dbg, sizeof(unsigned long long) * 160 * 512 * 8) == cudaSuccess ? 0 : -1;
+}
+#endif
 
 const char *rt_strerror(int code) {
   switch (code) {

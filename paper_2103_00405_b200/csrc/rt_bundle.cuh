@@ -13,10 +13,12 @@
 //   stream warps:  T_k += a_k * dt_prev      internal-time increment of the PREVIOUS firing (Eq.15)
 //                  dt_k = (P_k - T_k) / a_k  waiting time for THIS firing (Eq.24), +inf if a_k = 0
 //                  thread-local lexicographic min (Eq.25, ties to the lowest k)
-//   walker warp:   X += v_mu on this CTA's PRIVATE replica of X (Eq.5) -- every CTA knows mu
-//                  after the exchange, so X never crosses CTAs; redraw of P_mu (Eq.26); then the
-//                  dependency walk: stoich row of mu -> species record -> dense
-//                  dependency entries (k, reactants, sigma) -> new a_k for the k in [k0, k1).
+//   walker warp:   X += v_mu (Eq.5): every CTA knows mu after the exchange and applies the
+//                  update itself to the one L2-resident copy of X (versioned words, atomicMax:
+//                  see rt_device.cuh), so no CTA ever waits for another's write; redraw of
+//                  P_mu (Eq.26); then the dependency walk: 64-byte stoich row of
+//                  mu (with the dependency ranges of its species) -> dense 32-byte dependency
+//                  entries (k, reactants, sigma, c_k) -> new a_k for the k in [k0, k1).
 // The stream uses the OLD a_k, which is exactly the propensity that held during the elapsed
 // interval, so T is right for every k; only the waiting times of the refreshed reactions (and
 // of mu) are stale.  After one CTA barrier the new a_k / P_mu are stored, the threads that own
@@ -31,13 +33,17 @@ namespace rt {
 
 constexpr int kListCap = 1024;      // refreshed reactions a CTA stages per round
 constexpr int kWalkerWarps = 1;
+constexpr int kMaxBundleCtas = 160; // CTAs that may share one trajectory (5 exchange slots per lane)
+constexpr int kSlotStride = 32;     // u64 words between exchange slots: 256 B, so the 148 slots that every
+                                    // CTA polls spread over as many L2 slices instead of queueing on a few
 
 struct BundleParams {
   NetDev net;
   double *T, *P, *a;      // [B][M_pad]   (STATE_SMEM: written once, at the end of a trajectory)
   uint32_t *n;            // [B][M_pad]   firings per reaction
-  long long *X;           // [B][S][N]    one private replica of X per CTA
-  u64 *exch;              // [B][2][S][2] exchange slots, zeroed before launch
+  u64 *X;                 // [B][G][N]    versioned counts (rt_device.cuh); CTA r uses replica r % G
+  int G;                  //              so that no more than S/G CTAs hammer one L2 line
+  u64 *exch;              // [B][2][S][kSlotStride] exchange slots (2 words used), zeroed before launch
   int S, B;
   int pairs_per_cta;
   const long long *x0;    // [N]
@@ -51,6 +57,22 @@ struct BundleParams {
   int refresh_mode;       // 0 dependency walk, 1 recompute every a_k (the paper's GPU scheme)
   int *err;               // set to 1 on a barrier timeout
 };
+
+#ifdef RT_PHASE_TIMING
+#ifndef RT_PT_ALL
+#define RT_PT_ALL 0
+#endif
+constexpr bool getenv_all_ctas = RT_PT_ALL;
+__device__ unsigned long long g_dbg[160 * 512 * 8];   // [cta][firing][post, done, walk_done, stream_done] ns
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define PT_DECL long long pt_acc[6] = {0, 0, 0, 0, 0, 0}; long long pt_last = clock64();
+#define PT_G(slot) { if (gen < 512 && lane == 0) g_dbg[((size_t)r * 512 + gen) * 8 + (slot)] = gtime(); }
+#define PT_MARK(i) { long long now_ = clock64(); pt_acc[i] += now_ - pt_last; pt_last = now_; }
+#else
+#define PT_DECL
+#define PT_G(slot)
+#define PT_MARK(i)
+#endif
 
 constexpr long long kSpinLimitCycles = 6000000000ll;   // ~3 s: a barrier that long is a bug
 
@@ -67,13 +89,17 @@ struct BundleCtx {
 
 // Block-wide lexmin of the thread candidates, then all-gather of the S CTA partials through the
 // exchange slots (which is also the bundle barrier).  Every thread returns the bundle-wide
-// winner.  win.k == -2 signals a timeout.
+// winner.  win.k == -2 signals a timeout.  fence = true additionally orders all earlier global
+// writes of every CTA before all later reads of every CTA (start and end of a trajectory; the
+// per-firing call does not need it).
 template <int BLOCK>
 __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<BLOCK> &ctx,
-                                              u64 *exch, int r, uint32_t &gen, Cand mine) {
+                                              u64 *exch, const uint32_t *nfire, int r,
+                                              uint32_t &gen, Cand mine, bool fence, int &pf_k) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   mine = warp_lexmin(mine);
   if (lane == 0) ctx.warp_part[warp] = mine;
+  if (fence) __threadfence();
   __syncthreads();
   if (warp == 0) {
     Cand c = ctx.warp_part[lane];                 // BLOCK / 32 <= 32 partials
@@ -82,50 +108,81 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
     if (p.S > 1) {
       const uint32_t tag = gen + 1u;
       const u64 par = (u64)(((gen >> 1) & 1u) ^ 1u) << 63;     // never matches zeroed memory
-      u64 *buf = exch + (size_t)(gen & 1u) * (size_t)p.S * 2;
+      u64 *buf = exch + (size_t)(gen & 1u) * (size_t)p.S * kSlotStride;
+#ifdef RT_PHASE_TIMING
+      if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 0] = gtime();
+#endif
       if (lane == 0)
-        st_relaxed_v2(buf + 2 * r, (u64)__double_as_longlong(c.dt) | par,
+        st_relaxed_v2(buf + (size_t)kSlotStride * r, (u64)__double_as_longlong(c.dt) | par,
                       ((u64)tag << 32) | (u64)(uint32_t)c.k);
       c.dt = __longlong_as_double(0x7ff0000000000000ll);
       c.k = 0x7fffffff;
       const long long t0 = clock64();
-      for (int s = lane; s < p.S; s += 32) {
-        u64 w0, w1;
-        for (;;) {
-          ld_relaxed_v2(buf + 2 * s, w0, w1);
-          if ((uint32_t)(w1 >> 32) == tag && (w0 >> 63) == (par >> 63)) break;
-          if (clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); c.k = -2; break; }
-        }
-        if (c.k == -2) break;
-        const double dt = __longlong_as_double((long long)(w0 & 0x7fffffffffffffffull));
-        const int k = (int)(uint32_t)(w1 & 0x7fffffffu);
-        if (cand_less(dt, k, c)) { c.dt = dt; c.k = k; }
+      // Lane l gathers slots l, l+32, ...: all of its loads are in flight together, so the
+      // all-gather completes one L2 round trip after the last CTA has posted.
+      constexpr int kMaxPer = kMaxBundleCtas / 32;
+      unsigned pending = 0;
+      for (int i = 0; i < kMaxPer; ++i) if (lane + 32 * i < p.S) pending |= 1u << i;
+      while (pending) {
+        u64 w0[kMaxPer], w1[kMaxPer];
+#pragma unroll
+        for (int i = 0; i < kMaxPer; ++i)
+          if (pending & (1u << i)) ld_relaxed_v2(buf + (size_t)kSlotStride * (lane + 32 * i), w0[i], w1[i]);
+#pragma unroll
+        for (int i = 0; i < kMaxPer; ++i)
+          if ((pending & (1u << i)) && (uint32_t)(w1[i] >> 32) == tag && (w0[i] >> 63) == (par >> 63)) {
+            pending &= ~(1u << i);
+            const double dt = __longlong_as_double((long long)(w0[i] & 0x7fffffffffffffffull));
+            const int k = (int)(uint32_t)(w1[i] & 0x7fffffffu);
+            if (cand_less(dt, k, c)) { c.dt = dt; c.k = k; }
+          }
+        if (pending && clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); c.k = -2; break; }
       }
       const bool timed_out = __any_sync(0xffffffffu, c.k == -2);
+#ifdef RT_PHASE_TIMING
+      if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 1] = gtime();
+#endif
       c = warp_lexmin(c);
       if (timed_out) c.k = -2;
     }
     if (lane == 0) ctx.win = c;
+  } else if (warp == BLOCK / 32 - 1 && !fence) {
+    // Walker warp, idle during the exchange: if this CTA's candidate wins (it usually stays the
+    // candidate for many firings before it does), every CTA will need its stoich row, the
+    // dependency entries of its species and its firing counter right after the exchange, and
+    // they are cold (each reaction fires rarely).  Pull them into L2 now, once per candidate.
+    Cand c = ctx.warp_part[lane];
+    if (lane >= BLOCK / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
+    c = warp_lexmin(c);
+    if (c.k != pf_k && c.k < p.net.M) {
+      pf_k = c.k;
+      int4 ent = make_int4(-1, 0, 0, 0);
+      if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(p.net.srow) + (size_t)c.k * 4 + lane);
+      if (lane == 0) prefetch_l2(nfire + c.k);
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int j = __shfl_sync(0xffffffffu, ent.x, e);
+        const uint32_t lo = (uint32_t)__shfl_sync(0xffffffffu, ent.z, e);
+        const uint32_t hi = (uint32_t)__shfl_sync(0xffffffffu, ent.w, e);
+        if (j >= 0 && hi != 0xffffffffu)            // hubs stay hot by themselves
+          for (uint32_t i = lo + 4u * lane; i < hi; i += 128u)
+            prefetch_l2(reinterpret_cast<const char *>(p.net.dep) + (size_t)i * 32);
+      }
+    }
   }
   gen += 1u;
   __syncthreads();
+  if (fence) __threadfence();
   return ctx.win;
 }
 
-#ifdef RT_PHASE_TIMING
-#define PT_DECL long long pt_acc[6] = {0, 0, 0, 0, 0, 0}; long long pt_last = clock64();
-#define PT_MARK(i) { long long now_ = clock64(); pt_acc[i] += now_ - pt_last; pt_last = now_; }
-#else
-#define PT_DECL
-#define PT_MARK(i)
-#endif
 
 // The per-firing pass of one thread over the reactions it owns.  UPDATE: also apply the
 // internal-time increment T_k += a_k * dprev (first pass); otherwise read-only (re-scan).
 // FULL: recompute a_k from X for every k (refresh_mode 1).
 // Ownership: STATE_SMEM -- local index i = tid, tid+NT, ...; global state -- pair q0+tid, +NT, ...
 template <int NT, bool SMEM, bool UPDATE>
-__device__ __forceinline__ Cand scan_own(const NetDev &net, const long long *X, int tid, int k0, int k1,
+__device__ __forceinline__ Cand scan_own(const NetDev &net, const u64 *X, int tid, int k0, int k1,
                                          double *sT, const double *sP, double *sA,
                                          double *T, double *P, double *A, double dprev, bool full) {
   Cand best;
@@ -202,39 +259,93 @@ __device__ __forceinline__ int owner_thread(int k, int k0) {
 
 
 
-// New propensity of the reaction of dependency entry d = (k, j1, j2, sigma1 | sigma2 << 8 |
-// general << 16), same operation order as propensity().  `on` = false turns the entry into a
-// harmless dummy (index 0 everywhere) so that the loads of a batch can be issued together.
-__device__ __forceinline__ double propensity_dep(const NetDev &net, const long long *X, int4 d, bool on) {
-  const int k = on ? d.x : 0, j1 = on ? d.y : 0, j2 = (on && d.z >= 0) ? d.z : 0;
-  const double c = __ldg(net.rate + k);
-  const long long x1 = X[j1], x2 = X[j2];
-  double a = __dmul_rn(c, __ll2double_rn(binom(x1, d.w & 0xff)));
-  if (d.z >= 0) a = __dmul_rn(a, __ll2double_rn(binom(x2, (d.w >> 8) & 0xff)));
-  if (on && (d.w & 0x10000)) a = propensity(net, X, k);    // more than two reactants (rare)
+// One dependency entry (32 bytes, see NetDev::dep).
+struct DepEnt {
+  int4 d;      // k, j1, j2 or -1, sigma1 | sigma2 << 8 | general << 16
+  double c;    // c_k
+};
+__device__ __forceinline__ DepEnt load_dep(const NetDev &net, uint32_t idx) {
+  const char *base = reinterpret_cast<const char *>(net.dep) + (size_t)idx * 32;
+  DepEnt e;
+  e.d = __ldg(reinterpret_cast<const int4 *>(base));
+  e.c = __ldg(reinterpret_cast<const double *>(base + 16));
+  return e;
+}
+
+// New propensity of the reaction of entry e, same operation order as propensity().  Branch-free
+// (but for the rare general case) so that the loads of a whole batch issue together; lanes
+// without work pass a copy of a valid entry, whose loads coalesce with the valid lanes'.
+__device__ __forceinline__ double propensity_dep(const NetDev &net, const u64 *X, const DepEnt &e, bool on) {
+  const long long x1 = x_load(X, e.d.y);
+  const long long x2 = x_load(X, e.d.z >= 0 ? e.d.z : e.d.y);
+  double a = __dmul_rn(e.c, __ll2double_rn(binom(x1, e.d.w & 0xff)));
+  if (e.d.z >= 0) a = __dmul_rn(a, __ll2double_rn(binom(x2, (e.d.w >> 8) & 0xff)));
+  if (on && (e.d.w & 0x10000)) a = propensity(net, X, e.d.x);    // more than two reactants (rare)
   return a;
 }
 
-// Walker-warp state for one firing, uniform over the warp except my_lo / my_hi.
-struct Walk {
-  int n_e;               // changed species of the fired reaction
-  int e;                 // species being walked
-  bool entered;          // (i, hi) hold the range of species e
-  uint32_t i, hi;        // dependency entries of species e still to visit
-  uint32_t my_lo, my_hi; // lane l: range of species l (l < 32)
-  uint32_t e0;           // CSR row start (rows with more than 4 entries)
+// Up to four dependency ranges walked as one flat index space, 128 entries per step so that
+// the loads of a whole step (typically of the whole firing) are in flight together.
+struct Ranges {
+  uint32_t lo[4];
+  uint32_t end[4];   // inclusive prefix sums of the range lengths
 };
 
-// Dependency range of species j restricted (for hubs: to the reaction blocks touching [k0,k1)).
-__device__ __forceinline__ void species_range(const NetDev &net, int j, int k0, int k1,
-                                              uint32_t &lo, uint32_t &hi) {
-  const uint2 rec = __ldg(reinterpret_cast<const uint2 *>(net.sp_rec) + j);
-  lo = rec.x; hi = rec.y;
-  if (hi - lo > (uint32_t)net.big_deg && k1 > k0) {
-    const uint32_t *off = net.big_off + (size_t)__ldg(net.sp_big + j) * (size_t)(net.n_blk + 1);
+// Visits flat indices [f, end[3]) of rg; stages (k, new a_k) for every entry with k in [k0, k1).
+// Returns true when the staging list filled up before the end (f then tells where to resume).
+__device__ __forceinline__ bool walk_ranges(const NetDev &net, const u64 *X, const Ranges &rg,
+                                            uint32_t &f, int k0, int k1, int lane, int &n,
+                                            int *list_k, double *list_a) {
+  const uint32_t total = rg.end[3];
+  while (f < total) {
+    if (n + 128 > kListCap) return true;
+    DepEnt ent[4];
+    bool in[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint32_t fi = f + (uint32_t)(u * 32 + lane);
+      const bool valid = fi < total;
+      const int e = (fi >= rg.end[0]) + (fi >= rg.end[1]) + (fi >= rg.end[2]);
+      const uint32_t beg = e == 0 ? 0u : e == 1 ? rg.end[0] : e == 2 ? rg.end[1] : rg.end[2];
+      const uint32_t lo = e == 0 ? rg.lo[0] : e == 1 ? rg.lo[1] : e == 2 ? rg.lo[2] : rg.lo[3];
+      ent[u] = load_dep(net, valid ? lo + (fi - beg) : rg.lo[0]);   // dummy: a line others load too
+      in[u] = valid && ent[u].d.x >= k0 && ent[u].d.x < k1;
+    }
+    double an[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) an[u] = propensity_dep(net, X, ent[u], in[u]);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const unsigned m = __ballot_sync(0xffffffffu, in[u]);
+      if (in[u]) {
+        const int pos = n + __popc(m & ((1u << lane) - 1u));
+        list_k[pos] = ent[u].d.x;
+        list_a[pos] = an[u];
+      }
+      n += __popc(m);
+    }
+    f += 128u;
+  }
+  return false;
+}
+
+// Dependency range of a species given its (lo, hi) or, for hubs, (row of big_off, 0xffffffff):
+// hubs are narrowed to the reaction blocks touching [k0, k1).
+__device__ __forceinline__ void narrow_range(const NetDev &net, uint32_t &lo, uint32_t &hi, int k0, int k1) {
+  if (hi == 0xffffffffu) {
+    const uint32_t *off = net.big_off + (size_t)lo * (size_t)(net.n_blk + 1);
     lo = __ldg(off + (k0 >> net.blk_shift));
     hi = __ldg(off + ((k1 - 1) >> net.blk_shift) + 1);
   }
+}
+
+// X_j += v for one changed species at firing number `ver` (>= 1).  Returns the new count, or
+// -1 if it would leave [0, xmax] (nothing is written then).  `apply` = false: only compute.
+__device__ __forceinline__ long long x_peek(const u64 *Xv, int j, int v, u64 ver, long long xmax, bool &done) {
+  const u64 w = __ldcg(Xv + j);
+  done = x_version(w) == ver;                  // another CTA has already applied this firing
+  const long long x = done ? x_count(w) : x_count(w) + (long long)v;
+  return (x < 0 || x > xmax) ? -1 : x;
 }
 
 template <int BLOCK, bool SMEM>
@@ -257,8 +368,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   double *P = p.P + (size_t)b * net.M_pad;
   double *A = p.a + (size_t)b * net.M_pad;
   uint32_t *nfire = p.n + (size_t)b * net.M_pad;
-  long long *X = p.X + ((size_t)b * p.S + r) * (size_t)N;     // this CTA's replica
-  u64 *exch = p.exch + (size_t)b * 2 * p.S * 2;
+  const int xg = r % p.G;                                      // X replica of this CTA
+  u64 *X = p.X + ((size_t)b * p.G + xg) * (size_t)N;
+  u64 *exch = p.exch + (size_t)b * 2 * p.S * kSlotStride;
 
   const int pairs_total = net.M_pad / 2;
   const int q0 = min(r * p.pairs_per_cta, pairs_total);
@@ -269,17 +381,20 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   double *sA = sP + (SMEM ? 2 * p.pairs_per_cta : 0);
 
   uint32_t gen = 0;   // exchange generation, identical in every CTA of the bundle
+  int pf_k = -1;      // walker warp: candidate whose walk data was last prefetched
   dirty[tid] = 0;
   if (tid == 0) { ctx.abort_local = 0; ctx.list_n = 0; ctx.more = 0; ctx.p_k = -1; }
   __syncthreads();
+  Cand none; none.dt = INF; none.k = 0x7fffffff;
 
   for (u64 it = (u64)b; it < p.n_traj; it += (u64)p.B) {
     const u64 traj = p.traj_first + it;
     const bool tracing = (it == 0) && p.trace_cap > 0 && r == 0;
 
-    // ---- a-0: X replica = x0, then T = 0, P = E(k,0), a = a(X0), n = 0 for the own range
-    for (int j = tid; j < N; j += BLOCK) X[j] = p.x0[j];
-    __syncthreads();
+    // ---- a-0: X = x0 (slices, version 0), then T = 0, P = E(k,0), a = a(X0), n = 0 for the own range
+    for (int j = (r / p.G) * BLOCK + tid; j < N; j += ((p.S - xg + p.G - 1) / p.G) * BLOCK)
+      __stcg(X + j, x_pack(0ull, p.x0[j]));
+    if (bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, none, true, pf_k).k == -2) return;
     for (int k = k0 + tid; k < k1; k += BLOCK) {
       double a0 = 0.0, p0 = 0.0;
       if (k < M) {
@@ -300,9 +415,15 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
 
     for (;;) {   // one iteration per firing, plus one closing pass
       PT_MARK(5)
-      Walk w;
-      w.n_e = 0; w.e = 0; w.entered = false; w.i = 0; w.hi = 0; w.my_lo = 0; w.my_hi = 0; w.e0 = 0;
-      Cand best; best.dt = INF; best.k = 0x7fffffff;
+      // walker-warp state of this firing (uniform over the warp)
+      Ranges rg;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { rg.lo[e] = 0; rg.end[e] = 0; }
+      uint32_t w_f = 0;         // flat position inside rg
+      int w_e = 0, w_ne = 0;    // CSR rows (more than 4 changed species): species cursor / count
+      uint32_t w_e0 = 0;
+      bool w_csr = false;
+      Cand best = none;
 
       if (is_walker && mu_prev >= 0) {
         // ===== walker warp: discrete updates of the previous firing (a-6, a-7, a-8) =====
@@ -312,28 +433,53 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           c_old = nfire[mu_prev];
           p_old = SMEM ? sP[mu_prev - k0] : __ldcg(P + mu_prev);
         }
-        const int4 row_j = __ldg(reinterpret_cast<const int4 *>(net.srow_j) + mu_prev);
-        const int4 row_v = __ldg(reinterpret_cast<const int4 *>(net.srow_v) + mu_prev);
-        const bool ell = row_j.x != -2;       // -2: more than 4 entries, use the CSR row instead
-        if (ell) {
-          w.n_e = (row_v.x != 0) + (row_v.y != 0) + (row_v.z != 0) + (row_v.w != 0);
-        } else {
-          w.e0 = __ldg(net.stoich_ptr + mu_prev);
-          w.n_e = (int)(__ldg(net.stoich_ptr + mu_prev + 1) - w.e0);
-        }
-        for (int e = lane; e < w.n_e; e += 32) {     // a-6: X += v_mu (Eq.5), entry e by lane e%32
-          int j, v;
-          if (ell) {
-            j = e == 0 ? row_j.x : e == 1 ? row_j.y : e == 2 ? row_j.z : row_j.w;
-            v = e == 0 ? row_v.x : e == 1 ? row_v.y : e == 2 ? row_v.z : row_v.w;
-          } else {
-            j = __ldg(net.stoich_species + w.e0 + e);
-            v = __ldg(net.stoich_v + w.e0 + e);
+        int4 ent = make_int4(-1, 0, 0, 0);      // lane e < 4: (j, v, lo, hi) of the e-th changed species
+        if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(net.srow) + (size_t)mu_prev * 4 + lane);
+        w_csr = __shfl_sync(0xffffffffu, ent.x, 0) == -2;
+        PT_G(4)
+        if (!w_csr) {
+          // a-6: X += v_mu (Eq.5); nothing is written if any count would leave [0, xmax]
+          const bool active = ent.x >= 0;
+          bool done = false;
+          long long xn = 0;
+          uint32_t lo = 0, hi = 0;
+          if (active && !full && k1 > k0) {        // (hub: two loads, in flight with the X word)
+            lo = (uint32_t)ent.z; hi = (uint32_t)ent.w;
+            narrow_range(net, lo, hi, k0, k1);
           }
-          if (e < 32 && !full) species_range(net, j, k0, k1, w.my_lo, w.my_hi);
-          const long long x = X[j] + (long long)v;
-          if (x < 0 || x > net.xmax) ctx.abort_local = 1;
-          X[j] = x;
+          if (active) xn = x_peek(X, ent.x, ent.y, fired, net.xmax, done);
+          const bool bad = __any_sync(0xffffffffu, active && xn < 0);
+          PT_G(5)
+          if (bad) { if (lane == 0) ctx.abort_local = 1; }
+          else if (active && !done) atomicMax(X + ent.x, x_pack(fired, xn));
+          uint32_t acc = 0;
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            rg.lo[e] = __shfl_sync(0xffffffffu, lo, e);
+            acc += __shfl_sync(0xffffffffu, hi - lo, e);
+            rg.end[e] = acc;
+          }
+        } else {
+          // rows with more than 4 changed species: plain CSR walk (rare, correctness path)
+          w_e0 = __ldg(net.stoich_ptr + mu_prev);
+          w_ne = (int)(__ldg(net.stoich_ptr + mu_prev + 1) - w_e0);
+          bool bad_l = false;
+          for (int e = lane; e < w_ne; e += 32) {
+            bool done;
+            bad_l |= x_peek(X, __ldg(net.stoich_species + w_e0 + e), __ldg(net.stoich_v + w_e0 + e),
+                            fired, net.xmax, done) < 0;
+          }
+          if (__any_sync(0xffffffffu, bad_l)) {
+            if (lane == 0) ctx.abort_local = 1;
+          } else {
+            for (int e = lane; e < w_ne; e += 32) {
+              bool done;
+              const int j = __ldg(net.stoich_species + w_e0 + e);
+              const long long xn = x_peek(X, j, __ldg(net.stoich_v + w_e0 + e), fired, net.xmax, done);
+              if (!done) atomicMax(X + j, x_pack(fired, xn));
+            }
+          }
+          if (full || k1 <= k0) w_ne = 0;
         }
         if (lane == 0) {
           if (owner) {                           // a-7: new internal firing time of mu (Eq.26)
@@ -346,7 +492,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
             if (p.trace_t) p.trace_t[fired - 1] = t;
           }
         }
-        __syncwarp();                            // the replica's new counts are visible warp-wide
+        __syncwarp();                            // this warp's X updates precede its reads below
+        PT_G(6)
       }
       if (full && mu_prev >= 0) __syncthreads(); // full recompute reads the new X in the stream
 
@@ -357,46 +504,23 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           // ===== walker warp: dependency walk (a-1 for k in D(mu) that fall in [k0, k1)) =====
           int n = 0;
           bool more = false;
-          if (!full && k1 > k0) {
-            while (w.e < w.n_e) {
-              if (!w.entered) {
-                if (w.e < 32) {
-                  w.i = __shfl_sync(0xffffffffu, w.my_lo, w.e);
-                  w.hi = __shfl_sync(0xffffffffu, w.my_hi, w.e);
-                } else {
-                  species_range(net, __ldg(net.stoich_species + w.e0 + w.e), k0, k1, w.i, w.hi);
-                }
-                w.entered = true;
+          if (!w_csr) {
+            more = walk_ranges(net, X, rg, w_f, k0, k1, lane, n, list_k, list_a);
+          } else {
+            while (w_e < w_ne) {
+              if (w_f == 0) {                    // entering species w_e: fetch its range
+                const int j = __ldg(net.stoich_species + w_e0 + w_e);
+                const uint2 rec = __ldg(reinterpret_cast<const uint2 *>(net.sp_rec) + j);
+                uint32_t lo = rec.x, hi = rec.y;
+                if (hi - lo > (uint32_t)net.big_deg) { lo = (uint32_t)__ldg(net.sp_big + j); hi = 0xffffffffu; }
+                narrow_range(net, lo, hi, k0, k1);
+                rg.lo[0] = lo;
+                rg.end[0] = rg.end[1] = rg.end[2] = rg.end[3] = hi - lo;
               }
-              while (w.i < w.hi) {
-                if (n + 128 > kListCap) { more = true; break; }
-                int4 d[4];
-                bool in[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                  const uint32_t idx = w.i + (uint32_t)(u * 32 + lane);
-                  const bool valid = idx < w.hi;
-                  d[u] = __ldg(reinterpret_cast<const int4 *>(net.dep) + (valid ? idx : w.i));
-                  in[u] = valid && d[u].x >= k0 && d[u].x < k1;
-                }
-                double an[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) an[u] = propensity_dep(net, X, d[u], in[u]);
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                  const unsigned m = __ballot_sync(0xffffffffu, in[u]);
-                  if (in[u]) {
-                    const int pos = n + __popc(m & ((1u << lane) - 1u));
-                    list_k[pos] = d[u].x;
-                    list_a[pos] = an[u];
-                  }
-                  n += __popc(m);
-                }
-                w.i += 128u;
-              }
+              more = walk_ranges(net, X, rg, w_f, k0, k1, lane, n, list_k, list_a);
               if (more) break;
-              w.e += 1;
-              w.entered = false;
+              w_e += 1;
+              w_f = 0;
             }
           }
           if (lane == 0) { ctx.list_n = n; ctx.more = more ? 1 : 0; }
@@ -405,6 +529,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           best = scan_own<NT, SMEM, true>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, dprev, full);
         }
         PT_MARK(1)
+#ifdef RT_PHASE_TIMING
+        if (gen < 512 && first_round && (tid == 0 || tid == NT)) g_dbg[((size_t)r * 512 + gen) * 8 + (tid == NT ? 2 : 3)] = gtime();
+#endif
         __syncthreads();
         // ----- apply the staged refreshes; mark the owning threads for a re-scan
         const int n = ctx.list_n;
@@ -434,7 +561,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
 
       // ---- a-3 argmin over the bundle
       PT_MARK(3)
-      const Cand win = bundle_argmin<BLOCK>(p, ctx, exch, r, gen, best);
+      const Cand win = bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, best, false, pf_k);
       PT_MARK(4)
       if (win.k == -2) return;
 
@@ -449,6 +576,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         finishing = true;
         continue;
       }
+      if (fired >= kXMaxVersion) { status = RT_ERR_OVERFLOW; break; }   // firing counter exhausted
       t = __dadd_rn(t, delta);
       fired += 1;
       mu_prev = win.k;
@@ -460,17 +588,14 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     }
 
 #ifdef RT_PHASE_TIMING
-    if (tid == 0 && (r == 0 || r == p.S - 1 || r == p.S / 2))
-      printf("cta %d stream thread: updates/sync %.0f  stream %.0f  apply %.0f  rescan %.0f  argmin+exchange %.0f  stop %.0f cyc/firing\n",
-             r, (double)pt_acc[0] / fired, (double)pt_acc[1] / fired, (double)pt_acc[2] / fired,
-             (double)pt_acc[3] / fired, (double)pt_acc[4] / fired, (double)pt_acc[5] / fired);
-    if (tid == NT && (r == 0 || r == p.S - 1 || r == p.S / 2))
-      printf("cta %d walker: updates %.0f  walk %.0f  apply %.0f  rescan %.0f  argmin+exchange %.0f  stop %.0f cyc/firing\n",
-             r, (double)pt_acc[0] / fired, (double)pt_acc[1] / fired, (double)pt_acc[2] / fired,
+    if ((tid == 0 || tid == NT) && (getenv_all_ctas || r == 0 || r == p.S - 1 || r == p.S / 2))
+      printf("cta %d %s: updates %.0f  %s %.0f  barrier+apply %.0f  rescan %.0f  argmin+exchange %.0f  stop tests %.0f cyc/firing\n",
+             r, tid == 0 ? "stream thread" : "walker", (double)pt_acc[0] / fired,
+             tid == 0 ? "stream" : "walk", (double)pt_acc[1] / fired, (double)pt_acc[2] / fired,
              (double)pt_acc[3] / fired, (double)pt_acc[4] / fired, (double)pt_acc[5] / fired);
 #endif
-    // ---- trajectory done: write the state back (STATE_SMEM), X and the outcome
-    __syncthreads();
+    // ---- trajectory done: every CTA's X updates are visible bundle-wide after the fenced barrier
+    if (bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, none, true, pf_k).k == -2) return;
     dirty[tid] = 0;
     if (SMEM)
       for (int k = k0 + tid; k < k1; k += BLOCK) {
@@ -478,7 +603,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       }
     if (p.x_out)
       for (int j = r * BLOCK + tid; j < N; j += p.S * BLOCK)
-        p.x_out[it * (u64)N + (u64)j] = X[j];
+        p.x_out[it * (u64)N + (u64)j] = x_load(X, j);
     if (r == 0 && tid == 0) {
       rt_result res;
       res.t = t; res.firings = fired; res.stop = stop; res.status = status;

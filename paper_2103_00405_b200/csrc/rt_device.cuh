@@ -25,13 +25,16 @@ struct NetDev {
   const double *rate;            // [M]
   // Dependency graph, stored two-hop and dense so that a walk is three
   // dependent loads: stoich row of mu -> species record -> dependency entries.
-  const int32_t *srow_j;         // [M][4] changed species of reaction k (ELL copy of its stoich row;
-  const int32_t *srow_v;         // [M][4]  v = 0: unused slot; srow_j[k][0] = -2: row has > 4 entries)
+  const int32_t *srow;           // [M][4][4] ELL copy of the stoich row of k, 64 B: per changed species
+                                 //        (j, v, lo, hi): [lo, hi) = its entries in dep[]; hubs store
+                                 //        (j, v, row of big_off, 0xffffffff); unused slot j = -1;
+                                 //        srow[k][0].j = -2: more than 4 entries, walk the CSR row
   const uint32_t *sp_rec;        // [N][2] (lo, hi): entries of species j in dep[]
   const int32_t *sp_big;         // [N]    row of big_off for hub species (degree > big_deg), else -1
   const uint32_t *big_off;       // [n_big][n_blk+1] hub species: first entry with k >= b << blk_shift
-  const int32_t *dep;            // [nnz_r][4] (k, j1, j2 or -1, sigma1 | sigma2 << 8 | general << 16),
-                                 //        sorted by k within a species; (j1, j2) = first two reactants of k
+  const int32_t *dep;            // [nnz_r] 32-byte entries, sorted by k within a species:
+                                 //        int32 k, j1, j2 (or -1), sigma1 | sigma2 << 8 | general << 16;
+                                 //        double c_k; 8 bytes padding.  (j1, j2) = first two reactants
   int32_t n_blk, blk_shift, big_deg;
   long long xmax;                // count bound (2^31-1, or 2^21-1 if some sigma = 3)
 };
@@ -76,13 +79,28 @@ __device__ __forceinline__ long long binom(long long x, int sigma) {
   return h * (x - 2) / 3;
 }
 
+// The bundle kernel keeps ONE copy of X per trajectory in global memory (L2-resident), each
+// word = (version << 31) | count: version = index of the firing that last changed the species
+// (1-based, 33 bits), count < 2^31.  Every CTA applies every firing's update itself with
+// atomicMax (red.max.u64): all CTAs write the same word, and a delayed write of an older firing
+// can never replace a newer one, so no fence sits between a firing and the next.
+constexpr int kXCountBits = 31;
+constexpr u64 kXCountMask = (1ull << kXCountBits) - 1ull;
+constexpr u64 kXMaxVersion = (1ull << (64 - kXCountBits)) - 2ull;
+__device__ __forceinline__ long long x_count(u64 w) { return (long long)(w & kXCountMask); }
+__device__ __forceinline__ u64 x_version(u64 w) { return w >> kXCountBits; }
+__device__ __forceinline__ u64 x_pack(u64 version, long long count) {
+  return (version << kXCountBits) | (u64)count;
+}
+__device__ __forceinline__ long long x_load(const u64 *Xv, int j) { return x_count(__ldcg(Xv + j)); }
+
 // a_k = c_k * prod_j C(X_j, sigma_jk): one rounded multiply per reactant, CSR order.
-// X is the calling CTA's private replica (or shared memory), so plain loads are coherent.
-__device__ __forceinline__ double propensity(const NetDev &net, const long long *X, int k) {
+// X is read with ld.global.cg (L2): other CTAs write it too.
+__device__ __forceinline__ double propensity(const NetDev &net, const u64 *Xv, int k) {
   double a = __ldg(net.rate + k);
   const uint32_t e1 = __ldg(net.react_ptr + k + 1);
   for (uint32_t e = __ldg(net.react_ptr + k); e < e1; ++e) {
-    const long long x = X[__ldg(net.react_species + e)];
+    const long long x = x_load(Xv, __ldg(net.react_species + e));
     a = __dmul_rn(a, __ll2double_rn(binom(x, __ldg(net.react_sigma + e))));
   }
   return a;
@@ -122,6 +140,9 @@ __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {
   uint32_t v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
+}
+__device__ __forceinline__ void prefetch_l2(const void *p) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
 }
 __device__ __forceinline__ void st_relaxed_v2(u64 *p, u64 a, u64 b) {
   asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");

@@ -104,16 +104,17 @@ def test_hub_species_general_rows_and_staging_overflow(rt, ctas, state_mode):
 
 
 def test_count_overflow_is_reported(rt):
-    """0 -> X from the count bound: the first firing leaves [0, 2^31-1] -> RT_ERR_OVERFLOW."""
+    """0 -> X from the count bound: after the three deaths of the other species the first birth
+    leaves [0, 2^31-1] -> RT_ERR_OVERFLOW at firing 4."""
     net = W.from_reactions(2, [({}, {0: 1}, 1.0), ({1: 1}, {}, 1.0)])
     x0 = np.array([2**31 - 1, 3], dtype=np.int64)
     o = _oracle().run(net, x0, 5, 0, 100, math.inf, 100, check=False)
     with rt.Model(net) as m:
         g = m.run(x0, 5, 0, 100, math.inf, 100, check=False)
     assert g["code"] == rt.RT_ERR_OVERFLOW and g["status"] == rt.RT_ERR_OVERFLOW
-    assert g["firings"] == o["firings"]
-    np.testing.assert_array_equal(g["x"], o["x"])
+    assert o["code"] == -5 and g["firings"] == o["firings"] == 4
     np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
+    np.testing.assert_array_equal(g["x"], [2**31 - 1, 0])   # the offending update is not applied
 
 
 def test_cfg3_full_first_1e4(rt):
