@@ -138,15 +138,21 @@ int upload(DevBuf &buf, const std::vector<T> &host) {
 }
 
 // How one launch is shaped: B bundles of S CTAs; smem = the (T,P,a) state lives in shared memory.
-struct Plan { int S, B, G; int pairs_per_cta; bool smem; };
+struct Plan { int S, B, G; int pairs_per_cta; int cnt_pad; bool smem; };
 
-size_t smem_state_bytes(int pairs_per_cta) { return (size_t)pairs_per_cta * 2 * 3 * sizeof(double); }
+// slots per shared-memory state array: a CTA's reactions padded to whole scan batches
+int padded_count(int pairs_per_cta) {
+  const int batch = rt::kScanBatch * (kBlock - 32 * rt::kWalkerWarps);
+  return (2 * pairs_per_cta + batch - 1) / batch * batch;
+}
+size_t smem_state_bytes(int pairs_per_cta) { return (size_t)padded_count(pairs_per_cta) * 3 * sizeof(double); }
 
 Plan plan_bundles(const rt_model *m, u64 n_traj) {
   const int pairs_total = m->net.M_pad / 2;
   const int sms = m->num_sms;
   // fewest CTAs whose share of the state still fits in shared memory
-  const int pairs_fit = (int)(kSmemStateBytes / (2 * 3 * sizeof(double)));
+  const int batch = rt::kScanBatch * (kBlock - 32 * rt::kWalkerWarps);
+  const int pairs_fit = std::max(1, (int)(kSmemStateBytes / (3 * sizeof(double)) / batch * batch / 2));
   const int s_fit = (pairs_total + pairs_fit - 1) / pairs_fit;
   const int s_thin = std::max(1, (pairs_total + kMinPairsPerCta - 1) / kMinPairsPerCta);
   int S;
@@ -166,6 +172,7 @@ Plan plan_bundles(const rt_model *m, u64 n_traj) {
   pl.pairs_per_cta = (pairs_total + S - 1) / S;
   pl.G = std::min(S, m->opt_x_replicas > 0 ? m->opt_x_replicas : 1);      // X replicas: spread the per-firing reads/atomics of hot species
   while (pl.G > 1 && (size_t)pl.B * pl.G * (size_t)m->net.N * 8 > ((size_t)64 << 20)) pl.G /= 2;
+  pl.cnt_pad = padded_count(pl.pairs_per_cta);
   pl.smem = m->opt_state_mode != 1 && smem_state_bytes(pl.pairs_per_cta) <= kSmemStateBytes;
   return pl;
 }
@@ -195,7 +202,7 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.T = (double *)m->d_T.p; p.P = (double *)m->d_P.p; p.a = (double *)m->d_a.p;
   p.n = (uint32_t *)m->d_n.p; p.X = (u64 *)m->d_X.p;
   p.exch = (u64 *)m->d_exch.p;
-  p.S = pl.S; p.B = pl.B; p.G = pl.G; p.pairs_per_cta = pl.pairs_per_cta;
+  p.S = pl.S; p.B = pl.B; p.G = pl.G; p.pairs_per_cta = pl.pairs_per_cta; p.cnt_pad = pl.cnt_pad;
   p.x0 = x0_dev; p.seed = seed; p.traj_first = traj_first; p.n_traj = n_traj;
   p.max_firings = max_firings; p.t_end = t_end;
   p.x_out = x_out_dev; p.res = res_dev;
@@ -308,6 +315,7 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
       rg(net->react_sigma, net->react_sigma + nr), ss(net->stoich_species, net->stoich_species + nv),
       sv(net->stoich_v, net->stoich_v + nv);
   std::vector<double> rate(net->rate, net->rate + M);
+  for (double &c : rate) c += 0.0;     // -0.0 -> +0.0: a_k is then never -0.0 (same results: a_k = 0 either way)
   // ---- dependency graph, two-hop: stoich row of mu -> species -> reactions that
   // have the species as a reactant.  Entries of one species ascend in k (counting sort over the
   // reactant CSR, which is ordered by reaction) and carry what a refresh needs.

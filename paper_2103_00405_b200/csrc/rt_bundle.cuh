@@ -31,7 +31,7 @@
 
 namespace rt {
 
-constexpr int kListCap = 1024;      // refreshed reactions a CTA stages per round
+constexpr int kListCap = 512;       // refreshed reactions a CTA stages per round
 constexpr int kWalkerWarps = 1;
 constexpr int kMaxBundleCtas = 160; // CTAs that may share one trajectory (5 exchange slots per lane)
 constexpr int kSlotStride = 32;     // u64 words between exchange slots: 256 B, so the 148 slots that every
@@ -46,6 +46,8 @@ struct BundleParams {
   u64 *exch;              // [B][2][S][kSlotStride] exchange slots (2 words used), zeroed before launch
   int S, B;
   int pairs_per_cta;
+  int cnt_pad;            // STATE_SMEM: slots per array (the CTA's reactions padded to a whole number
+                          // of scan batches; padding slots hold a = T = 0, P = 1)
   const long long *x0;    // [N]
   u64 seed, traj_first, n_traj, max_firings;
   double t_end;
@@ -83,6 +85,7 @@ struct BundleCtx {
   int abort_local;        // a count left [0, xmax] (identical in every CTA: all replicate X)
   int list_n;             // staged refreshes of this round
   int more;               // walker has entries left for another round
+  int any_odd;            // some a_k of this CTA is outside the filter's safe range (sticky)
   int p_k;                // reaction whose P was redrawn (or -1), and its new value
   double p_val;
 };
@@ -177,6 +180,79 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
 }
 
 
+// ---- filtered scan (state in shared memory) ----------------------------------------------------
+// The argmin needs the correctly rounded quotient of only ONE of a thread's reactions: the others
+// are ruled out by an approximate quotient q~ = (float)(r * rcp.approx(a)).  rcp.approx.ftz.f64
+// (MUFU.RCP64H) is good to 2^-19.9 relative on normal inputs (measured over 4e9 values);
+// with the multiply's and the conversion's rounding q~ is within 2^-19.5 of the true quotient.
+// A reaction whose q~ exceeds (1 + 2^-16) times the thread's smallest q~ has a correctly rounded
+// quotient strictly above that reaction's, so it can neither win nor tie.  If a second reaction
+// of the thread is within the tolerance, or the smallest q~ is outside [2^-100, 2^100] (which
+// also catches negative residuals, zeros and NaNs), or some a_k of this CTA is outside the range
+// where the bound holds (`any_odd`), the thread divides exactly (__ddiv_rn) and compares
+// lexicographically -- so the result is always bit-identical to dividing everything.
+// a_k = 0 needs no test: rcp gives +inf, the product +inf or NaN, neither is ever the smallest.
+// Per reaction the pass issues ~16 instructions instead of ~45: the pass is issue-bound.
+constexpr float kFilterTol = 0x1.0p-16f;
+constexpr int kScanBatch = 4;     // reactions in flight per thread; state padded to kScanBatch * NT
+__device__ __forceinline__ double rcp_approx(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  return y;
+}
+// a_k values for which the error bound of the filter is not established (non-zero only)
+__device__ __forceinline__ bool filter_unsafe(double a) {
+  const unsigned ea = ((unsigned)__double2hiint(a) >> 20) & 0x7ffu;
+  return (ea - 100u >= 1847u) && ((__double_as_longlong(a) << 1) != 0ll);
+}
+
+template <int NT, bool UPDATE>
+__device__ __forceinline__ Cand scan_filtered(int tid, int k0, int cnt_pad, double *__restrict__ sT,
+                                              const double *__restrict__ sP,
+                                              const double *__restrict__ sA, double dprev, bool any_odd) {
+  constexpr int U = kScanBatch;
+  const float FINF = __int_as_float(0x7f800000);
+  float m1 = FINF, m2 = FINF;
+  int i1 = tid;
+  for (int i = tid; i < cnt_pad; i += U * NT) {
+    double a[U], t[U], pk[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) { a[u] = sA[i + u * NT]; t[u] = sT[i + u * NT]; pk[u] = sP[i + u * NT]; }
+    if (UPDATE) {
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        t[u] = __dadd_rn(t[u], __dmul_rn(a[u], dprev));
+        sT[i + u * NT] = t[u];
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const float q = __double2float_rn(__dmul_rn(__dsub_rn(pk[u], t[u]), rcp_approx(a[u])));
+      m2 = fminf(m2, fmaxf(q, m1));          // NaN (0 * inf) is dropped by fminf / fmaxf
+      if (q < m1) { m1 = q; i1 = i + u * NT; }
+    }
+  }
+  Cand best;
+  best.dt = __longlong_as_double(0x7ff0000000000000ll);
+  best.k = 0x7fffffff;
+  const float thr = m1 * (1.0f + kFilterTol);
+  if (!any_odd && m1 >= 0x1.0p-100f && m1 <= 0x1.0p100f && m2 > thr) {   // common case: one division
+    best.dt = waiting_time(sP[i1], sT[i1], sA[i1]);
+    best.k = k0 + i1;
+  } else {
+    const bool all = any_odd || !(m1 >= 0x1.0p-100f && m1 <= 0x1.0p100f);
+    for (int i = tid; i < cnt_pad; i += NT) {             // near tie (or odd values): a second,
+      const double a = sA[i], pk = sP[i], t = sT[i];      // read-only pass divides what is close
+      const float q = __double2float_rn(__dmul_rn(__dsub_rn(pk, t), rcp_approx(a)));
+      if (all || q <= thr) {
+        const double d = waiting_time(pk, t, a);
+        if (d < best.dt) { best.dt = d; best.k = k0 + i; }
+      }
+    }
+  }
+  return best;
+}
+
 // The per-firing pass of one thread over the reactions it owns.  UPDATE: also apply the
 // internal-time increment T_k += a_k * dprev (first pass); otherwise read-only (re-scan).
 // FULL: recompute a_k from X for every k (refresh_mode 1).
@@ -184,10 +260,12 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
 template <int NT, bool SMEM, bool UPDATE>
 __device__ __forceinline__ Cand scan_own(const NetDev &net, const u64 *X, int tid, int k0, int k1,
                                          double *sT, const double *sP, double *sA,
-                                         double *T, double *P, double *A, double dprev, bool full) {
+                                         double *T, double *P, double *A, double dprev, bool full,
+                                         int cnt_pad, bool any_odd) {
   Cand best;
   best.dt = __longlong_as_double(0x7ff0000000000000ll);
   best.k = 0x7fffffff;
+  if (SMEM && !full) return scan_filtered<NT, UPDATE>(tid, k0, cnt_pad, sT, sP, sA, dprev, any_odd);
   if (SMEM) {
     const int cnt = k1 - k0;
 #pragma unroll 4
@@ -272,15 +350,14 @@ __device__ __forceinline__ DepEnt load_dep(const NetDev &net, uint32_t idx) {
   return e;
 }
 
-// New propensity of the reaction of entry e, same operation order as propensity().  Branch-free
-// (but for the rare general case) so that the loads of a whole batch issue together; lanes
-// without work pass a copy of a valid entry, whose loads coalesce with the valid lanes'.
-__device__ __forceinline__ double propensity_dep(const NetDev &net, const u64 *X, const DepEnt &e, bool on) {
-  const long long x1 = x_load(X, e.d.y);
-  const long long x2 = x_load(X, e.d.z >= 0 ? e.d.z : e.d.y);
-  double a = __dmul_rn(e.c, __ll2double_rn(binom(x1, e.d.w & 0xff)));
-  if (e.d.z >= 0) a = __dmul_rn(a, __ll2double_rn(binom(x2, (e.d.w >> 8) & 0xff)));
-  if (on && (e.d.w & 0x10000)) a = propensity(net, X, e.d.x);    // more than two reactants (rare)
+// New propensity of the reaction of entry d = (k, j1, j2, sigma1 | sigma2 << 8 | general << 16)
+// with rate c: same operation order as propensity().
+__device__ __forceinline__ double propensity_dep(const NetDev &net, const u64 *X, const int4 d, double c) {
+  if (d.w & 0x10000) return propensity(net, X, d.x);    // more than two reactants (rare)
+  const long long x1 = x_load(X, d.y);
+  const long long x2 = x_load(X, d.z >= 0 ? d.z : d.y);
+  double a = __dmul_rn(c, __ll2double_rn(binom(x1, d.w & 0xff)));
+  if (d.z >= 0) a = __dmul_rn(a, __ll2double_rn(binom(x2, (d.w >> 8) & 0xff)));
   return a;
 }
 
@@ -291,11 +368,11 @@ struct Ranges {
   uint32_t end[4];   // inclusive prefix sums of the range lengths
 };
 
-// Visits flat indices [f, end[3]) of rg; stages (k, new a_k) for every entry with k in [k0, k1).
-// Returns true when the staging list filled up before the end (f then tells where to resume).
-__device__ __forceinline__ bool walk_ranges(const NetDev &net, const u64 *X, const Ranges &rg,
-                                            uint32_t &f, int k0, int k1, int lane, int &n,
-                                            int *list_k, double *list_a) {
+// Scan: visits flat indices [f, end[3]) of rg and compacts the entries with k in [k0, k1) into
+// (list_d, list_a = c_k).  Cheap per entry, so the many entries of other CTAs' reactions cost
+// little.  Returns true when the staging list filled up (f then tells where to resume).
+__device__ __forceinline__ bool walk_scan(const NetDev &net, const Ranges &rg, uint32_t &f, int k0,
+                                          int k1, int lane, int &n, int4 *list_d, double *list_a) {
   const uint32_t total = rg.end[3];
   while (f < total) {
     if (n + 128 > kListCap) return true;
@@ -308,25 +385,33 @@ __device__ __forceinline__ bool walk_ranges(const NetDev &net, const u64 *X, con
       const int e = (fi >= rg.end[0]) + (fi >= rg.end[1]) + (fi >= rg.end[2]);
       const uint32_t beg = e == 0 ? 0u : e == 1 ? rg.end[0] : e == 2 ? rg.end[1] : rg.end[2];
       const uint32_t lo = e == 0 ? rg.lo[0] : e == 1 ? rg.lo[1] : e == 2 ? rg.lo[2] : rg.lo[3];
-      ent[u] = load_dep(net, valid ? lo + (fi - beg) : rg.lo[0]);   // dummy: a line others load too
+      ent[u] = load_dep(net, valid ? lo + (fi - beg) : rg.lo[0]);   // idle lanes: a line others load too
       in[u] = valid && ent[u].d.x >= k0 && ent[u].d.x < k1;
     }
-    double an[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) an[u] = propensity_dep(net, X, ent[u], in[u]);
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const unsigned m = __ballot_sync(0xffffffffu, in[u]);
       if (in[u]) {
         const int pos = n + __popc(m & ((1u << lane) - 1u));
-        list_k[pos] = ent[u].d.x;
-        list_a[pos] = an[u];
+        list_d[pos] = ent[u].d;
+        list_a[pos] = ent[u].c;
       }
       n += __popc(m);
     }
     f += 128u;
   }
   return false;
+}
+
+// Finish: new a_k for the n compacted entries (X loads of 32 entries in flight together).
+__device__ __forceinline__ void walk_finish(const NetDev &net, const u64 *X, int lane, int n,
+                                            const int4 *list_d, int *list_k, double *list_a) {
+  __syncwarp();
+  for (int i = lane; i < n; i += 32) {
+    const int4 d = list_d[i];
+    list_k[i] = d.x;
+    list_a[i] = propensity_dep(net, X, d, list_a[i]);
+  }
 }
 
 // Dependency range of a species given its (lo, hi) or, for hubs, (row of big_off, 0xffffffff):
@@ -353,6 +438,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   constexpr int NT = BLOCK - 32 * kWalkerWarps;      // stream threads; the last warp walks
   __shared__ BundleCtx<BLOCK> ctx;
   __shared__ int list_k[kListCap];
+  __shared__ int4 list_d[kListCap];
   __shared__ double list_a[kListCap];
   __shared__ unsigned char dirty[BLOCK];
   extern __shared__ __align__(16) unsigned char dyn_smem[];
@@ -377,13 +463,14 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   const int q1 = min(q0 + p.pairs_per_cta, pairs_total);
   const int k0 = 2 * q0, k1 = 2 * q1;
   double *sT = reinterpret_cast<double *>(dyn_smem);
-  double *sP = sT + (SMEM ? 2 * p.pairs_per_cta : 0);
-  double *sA = sP + (SMEM ? 2 * p.pairs_per_cta : 0);
+  const int cnt_pad = p.cnt_pad;
+  double *sP = sT + (SMEM ? cnt_pad : 0);
+  double *sA = sP + (SMEM ? cnt_pad : 0);
 
   uint32_t gen = 0;   // exchange generation, identical in every CTA of the bundle
   int pf_k = -1;      // walker warp: candidate whose walk data was last prefetched
   dirty[tid] = 0;
-  if (tid == 0) { ctx.abort_local = 0; ctx.list_n = 0; ctx.more = 0; ctx.p_k = -1; }
+  if (tid == 0) { ctx.abort_local = 0; ctx.list_n = 0; ctx.more = 0; ctx.p_k = -1; ctx.any_odd = 0; }
   __syncthreads();
   Cand none; none.dt = INF; none.k = 0x7fffffff;
 
@@ -395,15 +482,16 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     for (int j = (r / p.G) * BLOCK + tid; j < N; j += ((p.S - xg + p.G - 1) / p.G) * BLOCK)
       __stcg(X + j, x_pack(0ull, p.x0[j]));
     if (bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, none, true, pf_k).k == -2) return;
-    for (int k = k0 + tid; k < k1; k += BLOCK) {
-      double a0 = 0.0, p0 = 0.0;
-      if (k < M) {
+    for (int k = k0 + tid; k < (SMEM ? k0 + cnt_pad : k1); k += BLOCK) {
+      double a0 = 0.0, p0 = 1.0;     // padding: a = 0, P - T = 1 > 0, so its q~ is +inf, never NaN
+      if (k < k1 && k < M) {
         a0 = propensity(net, X, k);
         p0 = exp_draw(p.seed, traj, (uint32_t)k, 0u);
+        if (filter_unsafe(a0)) ctx.any_odd = 1;
       }
       if (SMEM) { sT[k - k0] = 0.0; sP[k - k0] = p0; sA[k - k0] = a0; }
       else { __stcg(T + k, 0.0); __stcg(P + k, p0); __stcg(A + k, a0); }
-      nfire[k] = 0u;
+      if (k < k1) nfire[k] = 0u;
     }
     __syncthreads();
 
@@ -505,7 +593,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           int n = 0;
           bool more = false;
           if (!w_csr) {
-            more = walk_ranges(net, X, rg, w_f, k0, k1, lane, n, list_k, list_a);
+            more = walk_scan(net, rg, w_f, k0, k1, lane, n, list_d, list_a);
           } else {
             while (w_e < w_ne) {
               if (w_f == 0) {                    // entering species w_e: fetch its range
@@ -517,16 +605,18 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
                 rg.lo[0] = lo;
                 rg.end[0] = rg.end[1] = rg.end[2] = rg.end[3] = hi - lo;
               }
-              more = walk_ranges(net, X, rg, w_f, k0, k1, lane, n, list_k, list_a);
+              more = walk_scan(net, rg, w_f, k0, k1, lane, n, list_d, list_a);
               if (more) break;
               w_e += 1;
               w_f = 0;
             }
           }
+          walk_finish(net, X, lane, n, list_d, list_k, list_a);
           if (lane == 0) { ctx.list_n = n; ctx.more = more ? 1 : 0; }
         } else if (first_round) {
           // ===== stream warps: a-5 of the previous firing fused with a-2/a-3 of this one =====
-          best = scan_own<NT, SMEM, true>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, dprev, full);
+          best = scan_own<NT, SMEM, true>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, dprev, full, cnt_pad,
+                                          ctx.any_odd != 0);
         }
         PT_MARK(1)
 #ifdef RT_PHASE_TIMING
@@ -539,6 +629,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         for (int i = tid; i < n; i += BLOCK) {
           const int k = list_k[i];
           if (SMEM) sA[k - k0] = list_a[i]; else __stcg(A + k, list_a[i]);
+          if (SMEM && filter_unsafe(list_a[i])) ctx.any_odd = 1;
           dirty[owner_thread<NT, SMEM>(k, k0)] = 1;
         }
         if (tid == 0 && ctx.p_k >= 0) {
@@ -554,7 +645,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       PT_MARK(2)
       if (!is_walker && dirty[tid]) {            // re-scan (read-only) with the new a_k, P_mu
         dirty[tid] = 0;
-        best = scan_own<NT, SMEM, false>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, 0.0, false);
+        best = scan_own<NT, SMEM, false>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, 0.0, false, cnt_pad,
+                                         ctx.any_odd != 0);
       }
       if (ctx.abort_local) { status = RT_ERR_OVERFLOW; stop = 0; break; }
       if (finishing) break;
@@ -609,7 +701,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       res.t = t; res.firings = fired; res.stop = stop; res.status = status;
       p.res[it] = res;
     }
-    if (tid == 0) { ctx.abort_local = 0; ctx.p_k = -1; }
+    if (tid == 0) { ctx.abort_local = 0; ctx.p_k = -1; ctx.any_odd = 0; }
     __syncthreads();
   }
 }
