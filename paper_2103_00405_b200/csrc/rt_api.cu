@@ -72,7 +72,7 @@ struct rt_model {
   // staging for the host-pointer API
   DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t;
   // options
-  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0;
+  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0, opt_prefetch = 3;
   // info
   int64_t kernel_launches = 0;
   int last_S = 0, last_B = 0, last_path = 0, last_state_smem = 0;
@@ -209,6 +209,7 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.trace_mu = trace_mu_dev; p.trace_t = trace_t_dev;
   p.trace_cap = (trace_mu_dev || trace_t_dev) ? trace_cap : 0;
   p.refresh_mode = m->refresh_mode;
+  p.prefetch = m->opt_prefetch;
   p.err = (int *)m->d_err.p;
   void *args[] = {&p};
   // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
@@ -533,6 +534,9 @@ int rt_set_option(rt_model *m, const char *name, int64_t value) {
   } else if (!strcmp(name, "ensemble_path")) {
     if (value < 0 || value > 2) return RT_ERR_BAD_ARG;
     m->opt_ensemble_path = (int)value;
+  } else if (!strcmp(name, "prefetch")) {
+    if (value < 0 || value > 3) return RT_ERR_BAD_ARG;
+    m->opt_prefetch = (int)value;
   } else if (!strcmp(name, "x_replicas")) {
     if (value < 0 || value > 64) return RT_ERR_BAD_ARG;
     m->opt_x_replicas = (int)value;

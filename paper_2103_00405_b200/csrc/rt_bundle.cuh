@@ -56,6 +56,7 @@ struct BundleParams {
   int32_t *trace_mu;      // first trajectory of the launch only; may be nullptr
   double *trace_t;
   u64 trace_cap;
+  int prefetch;           // walker prefetches its candidate's walk data during the exchange
   int refresh_mode;       // 0 dependency walk, 1 recompute every a_k (the paper's GPU scheme)
   int *err;               // set to 1 on a barrier timeout
 };
@@ -67,9 +68,15 @@ struct BundleParams {
 constexpr bool getenv_all_ctas = RT_PT_ALL;
 __device__ unsigned long long g_dbg[160 * 512 * 8];   // [cta][firing][post, done, walk_done, stream_done] ns
 __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#if RT_PHASE_TIMING >= 2
 #define PT_DECL long long pt_acc[6] = {0, 0, 0, 0, 0, 0}; long long pt_last = clock64();
 #define PT_G(slot) { if (gen < 512 && lane == 0) g_dbg[((size_t)r * 512 + gen) * 8 + (slot)] = gtime(); }
 #define PT_MARK(i) { long long now_ = clock64(); pt_acc[i] += now_ - pt_last; pt_last = now_; }
+#else
+#define PT_DECL long long pt_acc[6] = {0, 0, 0, 0, 0, 0};
+#define PT_G(slot)
+#define PT_MARK(i)
+#endif
 #else
 #define PT_DECL
 #define PT_G(slot)
@@ -95,10 +102,23 @@ struct BundleCtx {
 // winner.  win.k == -2 signals a timeout.  fence = true additionally orders all earlier global
 // writes of every CTA before all later reads of every CTA (start and end of a trajectory; the
 // per-firing call does not need it).
+// Walker-warp state that outlives a firing: what it has prepared for this CTA's candidate.
+struct Spec {
+  int pf_k;          // candidate whose walk data was last prefetched into L2
+  int k;             // candidate whose redraw is precomputed (lane 0), or -1
+  uint32_t n;        //   its new firing count
+  double P;          //   its new internal firing time P_k + E(seed, traj, k, n)
+  const double *sP;  // shared-memory P (nullptr: state in global memory)
+  const double *P_glob;
+  int k0;
+  u64 seed, traj;
+};
+
 template <int BLOCK>
 __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<BLOCK> &ctx,
                                               u64 *exch, const uint32_t *nfire, int r,
-                                              uint32_t &gen, Cand mine, bool fence, int &pf_k) {
+                                              uint32_t &gen, Cand mine, bool fence, Spec &spec) {
+  constexpr int NT = BLOCK - 32 * kWalkerWarps;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   mine = warp_lexmin(mine);
   if (lane == 0) ctx.warp_part[warp] = mine;
@@ -142,7 +162,7 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
         if (pending && clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); c.k = -2; break; }
       }
       const bool timed_out = __any_sync(0xffffffffu, c.k == -2);
-#ifdef RT_PHASE_TIMING
+#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING >= 2
       if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 1] = gtime();
 #endif
       c = warp_lexmin(c);
@@ -150,18 +170,25 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
     }
     if (lane == 0) ctx.win = c;
   } else if (warp == BLOCK / 32 - 1 && !fence) {
-    // Walker warp, idle during the exchange: if this CTA's candidate wins (it usually stays the
-    // candidate for many firings before it does), every CTA will need its stoich row, the
-    // dependency entries of its species and its firing counter right after the exchange, and
-    // they are cold (each reaction fires rarely).  Pull them into L2 now, once per candidate.
+    // Walker warp, idle during the exchange.  If this CTA's candidate wins (it usually stays the
+    // candidate for many firings before it does), this CTA must redraw P_k (Philox + log, the
+    // longest serial piece of a firing) and every CTA will need the candidate's stoich row and
+    // the dependency entries of its species, all DRAM-cold (each reaction fires rarely).
+    // Do the redraw now, speculatively, and pull the rest into L2 -- once per candidate.
     Cand c = ctx.warp_part[lane];
     if (lane >= BLOCK / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
     c = warp_lexmin(c);
-    if (c.k != pf_k && c.k < p.net.M) {
-      pf_k = c.k;
+    if (c.k < p.net.M && c.k != spec.k && lane == 0 && (p.prefetch & 2)) {
+      const uint32_t n1 = nfire[c.k] + 1u;
+      const double pold = spec.sP ? spec.sP[c.k - spec.k0] : __ldcg(spec.P_glob + c.k);
+      spec.P = __dadd_rn(pold, exp_draw(spec.seed, spec.traj, (uint32_t)c.k, n1));
+      spec.n = n1;
+      spec.k = c.k;
+    }
+    if (c.k != spec.pf_k && c.k < p.net.M && (p.prefetch & 1)) {
+      spec.pf_k = c.k;
       int4 ent = make_int4(-1, 0, 0, 0);
       if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(p.net.srow) + (size_t)c.k * 4 + lane);
-      if (lane == 0) prefetch_l2(nfire + c.k);
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
         const int j = __shfl_sync(0xffffffffu, ent.x, e);
@@ -174,8 +201,16 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
     }
   }
   gen += 1u;
-  __syncthreads();
-  if (fence) __threadfence();
+  if (fence) {
+    __syncthreads();
+    __threadfence();
+  } else {
+    // The stream warps leave as soon as warp 0 has the winner; the walker warp, which may still
+    // be busy with its speculative work, pairs with warp 0 on a barrier of its own.
+    if (warp == 0) asm volatile("bar.arrive 2, 64;" ::: "memory");
+    if (warp == BLOCK / 32 - 1) asm volatile("bar.sync 2, 64;" ::: "memory");
+    else asm volatile("bar.sync 1, %0;" ::"r"(NT) : "memory");
+  }
   return ctx.win;
 }
 
@@ -209,7 +244,8 @@ __device__ __forceinline__ bool filter_unsafe(double a) {
 template <int NT, bool UPDATE>
 __device__ __forceinline__ Cand scan_filtered(int tid, int k0, int cnt_pad, double *__restrict__ sT,
                                               const double *__restrict__ sP,
-                                              const double *__restrict__ sA, double dprev, bool any_odd) {
+                                              const double *__restrict__ sA, double dprev, bool any_odd,
+                                              bool &defer) {
   constexpr int U = kScanBatch;
   const float FINF = __int_as_float(0x7f800000);
   float m1 = FINF, m2 = FINF;
@@ -239,6 +275,11 @@ __device__ __forceinline__ Cand scan_filtered(int tid, int k0, int cnt_pad, doub
   if (!any_odd && m1 >= 0x1.0p-100f && m1 <= 0x1.0p100f && m2 > thr) {   // common case: one division
     best.dt = waiting_time(sP[i1], sT[i1], sA[i1]);
     best.k = k0 + i1;
+  } else if (UPDATE) {
+    // Not decidable by the filter.  In the first pass that is nearly always the thread that owns
+    // the reaction that just fired (its residual is ~0 until P is redrawn) -- which re-scans
+    // anyway once the new values are stored.  Leave every such case to the re-scan.
+    defer = true;
   } else {
     const bool all = any_odd || !(m1 >= 0x1.0p-100f && m1 <= 0x1.0p100f);
     for (int i = tid; i < cnt_pad; i += NT) {             // near tie (or odd values): a second,
@@ -261,11 +302,11 @@ template <int NT, bool SMEM, bool UPDATE>
 __device__ __forceinline__ Cand scan_own(const NetDev &net, const u64 *X, int tid, int k0, int k1,
                                          double *sT, const double *sP, double *sA,
                                          double *T, double *P, double *A, double dprev, bool full,
-                                         int cnt_pad, bool any_odd) {
+                                         int cnt_pad, bool any_odd, bool &defer) {
   Cand best;
   best.dt = __longlong_as_double(0x7ff0000000000000ll);
   best.k = 0x7fffffff;
-  if (SMEM && !full) return scan_filtered<NT, UPDATE>(tid, k0, cnt_pad, sT, sP, sA, dprev, any_odd);
+  if (SMEM && !full) return scan_filtered<NT, UPDATE>(tid, k0, cnt_pad, sT, sP, sA, dprev, any_odd, defer);
   if (SMEM) {
     const int cnt = k1 - k0;
 #pragma unroll 4
@@ -468,7 +509,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   double *sA = sP + (SMEM ? cnt_pad : 0);
 
   uint32_t gen = 0;   // exchange generation, identical in every CTA of the bundle
-  int pf_k = -1;      // walker warp: candidate whose walk data was last prefetched
+  Spec spec;
+  spec.pf_k = -1; spec.k = -1; spec.n = 0u; spec.P = 0.0;
+  spec.sP = nullptr; spec.P_glob = nullptr; spec.k0 = 0; spec.seed = p.seed; spec.traj = 0;
   dirty[tid] = 0;
   if (tid == 0) { ctx.abort_local = 0; ctx.list_n = 0; ctx.more = 0; ctx.p_k = -1; ctx.any_odd = 0; }
   __syncthreads();
@@ -476,12 +519,13 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
 
   for (u64 it = (u64)b; it < p.n_traj; it += (u64)p.B) {
     const u64 traj = p.traj_first + it;
+    spec.k = -1; spec.traj = traj; spec.sP = SMEM ? sP : nullptr; spec.P_glob = P; spec.k0 = k0;
     const bool tracing = (it == 0) && p.trace_cap > 0 && r == 0;
 
     // ---- a-0: X = x0 (slices, version 0), then T = 0, P = E(k,0), a = a(X0), n = 0 for the own range
     for (int j = (r / p.G) * BLOCK + tid; j < N; j += ((p.S - xg + p.G - 1) / p.G) * BLOCK)
       __stcg(X + j, x_pack(0ull, p.x0[j]));
-    if (bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, none, true, pf_k).k == -2) return;
+    if (bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, none, true, spec).k == -2) return;
     for (int k = k0 + tid; k < (SMEM ? k0 + cnt_pad : k1); k += BLOCK) {
       double a0 = 0.0, p0 = 1.0;     // padding: a = 0, P - T = 1 > 0, so its q~ is +inf, never NaN
       if (k < k1 && k < M) {
@@ -503,6 +547,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
 
     for (;;) {   // one iteration per firing, plus one closing pass
       PT_MARK(5)
+#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING >= 2
+      if (tid == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 7] = gtime();
+#endif
       // walker-warp state of this firing (uniform over the warp)
       Ranges rg;
 #pragma unroll
@@ -517,7 +564,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         // ===== walker warp: discrete updates of the previous firing (a-6, a-7, a-8) =====
         const bool owner = (mu_prev >= k0 && mu_prev < k1);
         uint32_t c_old = 0; double p_old = 0.0;
-        if (owner && lane == 0) {
+        const bool have_spec = (spec.k == mu_prev);          // lane 0: redraw precomputed
+        if (owner && lane == 0 && !have_spec) {
           c_old = nfire[mu_prev];
           p_old = SMEM ? sP[mu_prev - k0] : __ldcg(P + mu_prev);
         }
@@ -571,9 +619,15 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         }
         if (lane == 0) {
           if (owner) {                           // a-7: new internal firing time of mu (Eq.26)
-            nfire[mu_prev] = c_old + 1u;
-            ctx.p_val = __dadd_rn(p_old, exp_draw(p.seed, traj, (uint32_t)mu_prev, c_old + 1u));
+            if (have_spec) {
+              nfire[mu_prev] = spec.n;
+              ctx.p_val = spec.P;
+            } else {
+              nfire[mu_prev] = c_old + 1u;
+              ctx.p_val = __dadd_rn(p_old, exp_draw(p.seed, traj, (uint32_t)mu_prev, c_old + 1u));
+            }
             ctx.p_k = mu_prev;
+            spec.k = -1;
           }
           if (tracing && fired - 1 < p.trace_cap) {   // a-8
             if (p.trace_mu) p.trace_mu[fired - 1] = mu_prev;
@@ -615,17 +669,22 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           if (lane == 0) { ctx.list_n = n; ctx.more = more ? 1 : 0; }
         } else if (first_round) {
           // ===== stream warps: a-5 of the previous firing fused with a-2/a-3 of this one =====
+          bool defer = false;
           best = scan_own<NT, SMEM, true>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, dprev, full, cnt_pad,
-                                          ctx.any_odd != 0);
+                                          ctx.any_odd != 0, defer);
+          if (defer) dirty[tid] = 1;
         }
         PT_MARK(1)
-#ifdef RT_PHASE_TIMING
+#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING >= 2
         if (gen < 512 && first_round && (tid == 0 || tid == NT)) g_dbg[((size_t)r * 512 + gen) * 8 + (tid == NT ? 2 : 3)] = gtime();
 #endif
         __syncthreads();
         // ----- apply the staged refreshes; mark the owning threads for a re-scan
         const int n = ctx.list_n;
         const bool more = ctx.more != 0;
+#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING == 1
+        if (tid == 0 && gen < 512 && first_round) g_dbg[((size_t)r * 512 + gen) * 8 + 2] = (unsigned long long)n;
+#endif
         for (int i = tid; i < n; i += BLOCK) {
           const int k = list_k[i];
           if (SMEM) sA[k - k0] = list_a[i]; else __stcg(A + k, list_a[i]);
@@ -645,15 +704,16 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       PT_MARK(2)
       if (!is_walker && dirty[tid]) {            // re-scan (read-only) with the new a_k, P_mu
         dirty[tid] = 0;
+        bool defer = false;
         best = scan_own<NT, SMEM, false>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, 0.0, false, cnt_pad,
-                                         ctx.any_odd != 0);
+                                         ctx.any_odd != 0, defer);
       }
       if (ctx.abort_local) { status = RT_ERR_OVERFLOW; stop = 0; break; }
       if (finishing) break;
 
       // ---- a-3 argmin over the bundle
       PT_MARK(3)
-      const Cand win = bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, best, false, pf_k);
+      const Cand win = bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, best, false, spec);
       PT_MARK(4)
       if (win.k == -2) return;
 
@@ -679,7 +739,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       }
     }
 
-#ifdef RT_PHASE_TIMING
+#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING >= 2
     if ((tid == 0 || tid == NT) && (getenv_all_ctas || r == 0 || r == p.S - 1 || r == p.S / 2))
       printf("cta %d %s: updates %.0f  %s %.0f  barrier+apply %.0f  rescan %.0f  argmin+exchange %.0f  stop tests %.0f cyc/firing\n",
              r, tid == 0 ? "stream thread" : "walker", (double)pt_acc[0] / fired,
@@ -687,7 +747,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
              (double)pt_acc[3] / fired, (double)pt_acc[4] / fired, (double)pt_acc[5] / fired);
 #endif
     // ---- trajectory done: every CTA's X updates are visible bundle-wide after the fenced barrier
-    if (bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, none, true, pf_k).k == -2) return;
+    if (bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, none, true, spec).k == -2) return;
     dirty[tid] = 0;
     if (SMEM)
       for (int k = k0 + tid; k < k1; k += BLOCK) {
