@@ -213,16 +213,15 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.err = (int *)m->d_err.p;
   void *args[] = {&p};
   // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
-  if (pl.smem) {
-    const size_t dyn = smem_state_bytes(pl.pairs_per_cta);
-    CU_TRY(cudaFuncSetAttribute(rt::rt_bundle_kernel<kBlock, true>,
-                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-    CU_TRY(cudaLaunchCooperativeKernel((const void *)rt::rt_bundle_kernel<kBlock, true>,
-                                       dim3(pl.S * pl.B), dim3(kBlock), args, dyn, st));
-  } else {
-    CU_TRY(cudaLaunchCooperativeKernel((const void *)rt::rt_bundle_kernel<kBlock, false>,
-                                       dim3(pl.S * pl.B), dim3(kBlock), args, 0, st));
-  }
+  const void *kern;
+  if (pl.smem) kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlock, true, true>
+                                      : (const void *)rt::rt_bundle_kernel<kBlock, true, false>;
+  else kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlock, false, true>
+                              : (const void *)rt::rt_bundle_kernel<kBlock, false, false>;
+  const size_t dyn = pl.smem ? smem_state_bytes(pl.pairs_per_cta) : 0;
+  if (dyn) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+  // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
+  CU_TRY(cudaLaunchCooperativeKernel(kern, dim3(pl.S * pl.B), dim3(kBlock), args, dyn, st));
   m->kernel_launches += 1;
   m->last_S = pl.S; m->last_B = pl.B; m->last_path = 2; m->last_state_smem = pl.smem ? 1 : 0;
   return RT_OK;

@@ -474,7 +474,39 @@ __device__ __forceinline__ long long x_peek(const u64 *Xv, int j, int v, u64 ver
   return (x < 0 || x > xmax) ? -1 : x;
 }
 
-template <int BLOCK, bool SMEM>
+// Fenced barrier over the CTAs of a bundle (start and end of a trajectory): all earlier global
+// writes of every CTA are visible to all later reads of every CTA.  Uses the exchange slots and
+// generation counter of bundle_argmin.  Returns false on a timeout.
+template <int BLOCK>
+__device__ __noinline__ bool bundle_barrier(u64 *exch, int S, int r, uint32_t gen, int *err) {
+  __threadfence();
+  __syncthreads();
+  bool ok = true;
+  if (threadIdx.x < 32 && S > 1) {
+    const int lane = threadIdx.x;
+    const uint32_t tag = gen + 1u;
+    const u64 par = (u64)(((gen >> 1) & 1u) ^ 1u) << 63;
+    u64 *buf = exch + (size_t)(gen & 1u) * (size_t)S * kSlotStride;
+    if (lane == 0) st_relaxed_v2(buf + (size_t)kSlotStride * r, par | 0x7ff0000000000000ull, ((u64)tag << 32) | 0x7fffffffull);
+    const long long t0 = clock64();
+    for (int s = lane; s < S; s += 32) {
+      u64 w0, w1;
+      for (;;) {
+        ld_relaxed_v2(buf + (size_t)kSlotStride * s, w0, w1);
+        if ((uint32_t)(w1 >> 32) == tag && (w0 >> 63) == (par >> 63)) break;
+        if (clock64() - t0 > kSpinLimitCycles) { atomicExch(err, 1); ok = false; break; }
+      }
+      if (!ok) break;
+    }
+  }
+  ok = __syncthreads_and(ok ? 1 : 0) != 0;
+  __threadfence();
+  return ok;
+}
+
+// FULL = refresh_mode 1 (recompute every a_k each firing, the paper's own GPU scheme) is a separate
+// instantiation so that its code stays out of the instruction stream of the default kernel.
+template <int BLOCK, bool SMEM, bool FULL>
 __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams p) {
   constexpr int NT = BLOCK - 32 * kWalkerWarps;      // stream threads; the last warp walks
   __shared__ BundleCtx<BLOCK> ctx;
@@ -525,7 +557,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     // ---- a-0: X = x0 (slices, version 0), then T = 0, P = E(k,0), a = a(X0), n = 0 for the own range
     for (int j = (r / p.G) * BLOCK + tid; j < N; j += ((p.S - xg + p.G - 1) / p.G) * BLOCK)
       __stcg(X + j, x_pack(0ull, p.x0[j]));
-    if (bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, none, true, spec).k == -2) return;
+    if (!bundle_barrier<BLOCK>(exch, p.S, r, gen, p.err)) return;
+    gen += 1u;
     for (int k = k0 + tid; k < (SMEM ? k0 + cnt_pad : k1); k += BLOCK) {
       double a0 = 0.0, p0 = 1.0;     // padding: a = 0, P - T = 1 > 0, so its q~ is +inf, never NaN
       if (k < k1 && k < M) {
@@ -543,7 +576,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     u64 fired = 0;
     int mu_prev = -1, stop = 0, status = RT_OK;
     bool finishing = false;
-    const bool full = (p.refresh_mode != 0);
+    constexpr bool full = FULL;
 
     for (;;) {   // one iteration per firing, plus one closing pass
       PT_MARK(5)
@@ -747,7 +780,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
              (double)pt_acc[3] / fired, (double)pt_acc[4] / fired, (double)pt_acc[5] / fired);
 #endif
     // ---- trajectory done: every CTA's X updates are visible bundle-wide after the fenced barrier
-    if (bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, none, true, spec).k == -2) return;
+    if (!bundle_barrier<BLOCK>(exch, p.S, r, gen, p.err)) return;
+    gen += 1u;
     dirty[tid] = 0;
     if (SMEM)
       for (int k = k0 + tid; k < k1; k += BLOCK) {

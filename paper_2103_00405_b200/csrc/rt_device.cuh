@@ -62,7 +62,9 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 // n-th unit-exponential increment of channel k (Eq.23: Delta T = ln(1/r)).
 // key = (lo32 seed, hi32 seed), counter = (k, n, lo32 traj, hi32 traj);
 // r = (u53 + 1) * 2^-53 in (0, 1].
-__device__ __forceinline__ double exp_draw(u64 seed, u64 traj, uint32_t k, uint32_t n) {
+// (not inlined: Philox + log is ~4 KB of code, and the per-firing loop has to stay in the
+// instruction cache)
+__device__ __noinline__ double exp_draw(u64 seed, u64 traj, uint32_t k, uint32_t n) {
   uint32_t w0, w1;
   philox4x32_10(k, n, (uint32_t)traj, (uint32_t)(traj >> 32), (uint32_t)seed,
                 (uint32_t)(seed >> 32), w0, w1);
@@ -95,15 +97,21 @@ __device__ __forceinline__ u64 x_pack(u64 version, long long count) {
 __device__ __forceinline__ long long x_load(const u64 *Xv, int j) { return x_count(__ldcg(Xv + j)); }
 
 // a_k = c_k * prod_j C(X_j, sigma_jk): one rounded multiply per reactant, CSR order.
-// X is read with ld.global.cg (L2): other CTAs write it too.
-__device__ __forceinline__ double propensity(const NetDev &net, const u64 *Xv, int k) {
-  double a = __ldg(net.rate + k);
-  const uint32_t e1 = __ldg(net.react_ptr + k + 1);
-  for (uint32_t e = __ldg(net.react_ptr + k); e < e1; ++e) {
-    const long long x = x_load(Xv, __ldg(net.react_species + e));
-    a = __dmul_rn(a, __ll2double_rn(binom(x, __ldg(net.react_sigma + e))));
+// X is read with ld.global.cg (L2): other CTAs write it too.  Not inlined (code size); takes the
+// arrays rather than the NetDev so that no copy of the kernel parameters is forced into local memory.
+__device__ __noinline__ double propensity_csr(const double *rate, const uint32_t *react_ptr,
+                                              const int32_t *react_species, const int32_t *react_sigma,
+                                              const u64 *Xv, int k) {
+  double a = __ldg(rate + k);
+  const uint32_t e1 = __ldg(react_ptr + k + 1);
+  for (uint32_t e = __ldg(react_ptr + k); e < e1; ++e) {
+    const long long x = x_load(Xv, __ldg(react_species + e));
+    a = __dmul_rn(a, __ll2double_rn(binom(x, __ldg(react_sigma + e))));
   }
   return a;
+}
+__device__ __forceinline__ double propensity(const NetDev &net, const u64 *Xv, int k) {
+  return propensity_csr(net.rate, net.react_ptr, net.react_species, net.react_sigma, Xv, k);
 }
 
 // ------------------------------------------------------------------ lexicographic argmin
@@ -114,14 +122,19 @@ struct Cand {
 __device__ __forceinline__ bool cand_less(double dt, int k, const Cand &b) {
   return dt < b.dt || (dt == b.dt && k < b.k);
 }
+// Warp-wide lexicographic min of (dt, k), result in every lane.  dt >= 0 (or +inf), never NaN, so
+// its bit pattern orders like an unsigned integer: three REDUX.MIN steps (high word, low word
+// among the lanes that tie on the high word, k among the lanes that tie on both) replace five
+// rounds of 64-bit shuffles.
 __device__ __forceinline__ Cand warp_lexmin(Cand c) {
-#pragma unroll
-  for (int off = 16; off > 0; off >>= 1) {
-    const double odt = __shfl_xor_sync(0xffffffffu, c.dt, off);
-    const int ok = __shfl_xor_sync(0xffffffffu, c.k, off);
-    if (cand_less(odt, ok, c)) { c.dt = odt; c.k = ok; }
-  }
-  return c;
+  const unsigned hi = (unsigned)__double2hiint(c.dt), lo = (unsigned)__double2loint(c.dt);
+  const unsigned h = __reduce_min_sync(0xffffffffu, hi);
+  const unsigned l = __reduce_min_sync(0xffffffffu, hi == h ? lo : 0xffffffffu);
+  const unsigned k = __reduce_min_sync(0xffffffffu, (hi == h && lo == l) ? (unsigned)c.k : 0xffffffffu);
+  Cand r;
+  r.dt = __hiloint2double((int)h, (int)l);
+  r.k = (int)k;
+  return r;
 }
 
 // Waiting time of one channel (Eq.24 with constant a_k; readings G4, G7): a = 0 gives +inf.
