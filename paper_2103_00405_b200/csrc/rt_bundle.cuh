@@ -325,45 +325,38 @@ __device__ __forceinline__ Cand scan_own(const NetDev &net, const u64 *X, int ti
       if (d < best.dt) { best.dt = d; best.k = k0 + i; }
     }
   } else {
+    // State streamed from global memory (HBM regime): 4 pairs of reactions per thread and
+    // iteration, i.e. twelve 16-byte loads (192 B) in flight per thread before any is used.
     double2 *T2 = reinterpret_cast<double2 *>(T);
     double2 *P2 = reinterpret_cast<double2 *>(P);
     double2 *A2 = reinterpret_cast<double2 *>(A);
+    constexpr int U = 4;
     const int q0 = k0 >> 1, q1 = k1 >> 1;
-    for (int q = q0 + tid; q < q1; q += 2 * NT) {
-      const int qb = q + NT;
-      const bool hb = qb < q1;
-      double2 ta = __ldcg(T2 + q), pa = __ldcg(P2 + q), aa = __ldcg(A2 + q);
-      double2 tb, pb, ab;
-      if (hb) { tb = __ldcg(T2 + qb); pb = __ldcg(P2 + qb); ab = __ldcg(A2 + qb); }
-      if (UPDATE) {
-        ta.x = __dadd_rn(ta.x, __dmul_rn(aa.x, dprev));
-        ta.y = __dadd_rn(ta.y, __dmul_rn(aa.y, dprev));
-        __stcg(T2 + q, ta);
-        if (full) {
-          aa.x = (2 * q < net.M) ? propensity(net, X, 2 * q) : 0.0;
-          aa.y = (2 * q + 1 < net.M) ? propensity(net, X, 2 * q + 1) : 0.0;
-          __stcg(A2 + q, aa);
-        }
+    for (int q = q0 + tid; q < q1; q += U * NT) {
+      double2 tt[U], pp[U], aa[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int qu = q + u * NT;
+        if (qu < q1) { tt[u] = __ldcg(T2 + qu); pp[u] = __ldcg(P2 + qu); aa[u] = __ldcg(A2 + qu); }
+        else { tt[u] = make_double2(0.0, 0.0); pp[u] = tt[u]; aa[u] = tt[u]; }   // a = 0: no candidate
       }
-      double d = waiting_time(pa.x, ta.x, aa.x);
-      if (d < best.dt) { best.dt = d; best.k = 2 * q; }
-      d = waiting_time(pa.y, ta.y, aa.y);
-      if (d < best.dt) { best.dt = d; best.k = 2 * q + 1; }
-      if (hb) {
-        if (UPDATE) {
-          tb.x = __dadd_rn(tb.x, __dmul_rn(ab.x, dprev));
-          tb.y = __dadd_rn(tb.y, __dmul_rn(ab.y, dprev));
-          __stcg(T2 + qb, tb);
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int qu = q + u * NT;
+        if (UPDATE && qu < q1) {
+          tt[u].x = __dadd_rn(tt[u].x, __dmul_rn(aa[u].x, dprev));
+          tt[u].y = __dadd_rn(tt[u].y, __dmul_rn(aa[u].y, dprev));
+          __stcg(T2 + qu, tt[u]);
           if (full) {
-            ab.x = (2 * qb < net.M) ? propensity(net, X, 2 * qb) : 0.0;
-            ab.y = (2 * qb + 1 < net.M) ? propensity(net, X, 2 * qb + 1) : 0.0;
-            __stcg(A2 + qb, ab);
+            aa[u].x = (2 * qu < net.M) ? propensity(net, X, 2 * qu) : 0.0;
+            aa[u].y = (2 * qu + 1 < net.M) ? propensity(net, X, 2 * qu + 1) : 0.0;
+            __stcg(A2 + qu, aa[u]);
           }
         }
-        d = waiting_time(pb.x, tb.x, ab.x);
-        if (d < best.dt) { best.dt = d; best.k = 2 * qb; }
-        d = waiting_time(pb.y, tb.y, ab.y);
-        if (d < best.dt) { best.dt = d; best.k = 2 * qb + 1; }
+        double d = waiting_time(pp[u].x, tt[u].x, aa[u].x);
+        if (d < best.dt) { best.dt = d; best.k = 2 * qu; }
+        d = waiting_time(pp[u].y, tt[u].y, aa[u].y);
+        if (d < best.dt) { best.dt = d; best.k = 2 * qu + 1; }
       }
     }
   }
