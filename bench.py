@@ -31,9 +31,10 @@ import rt_workloads as W
 METRIC = "reaction firings/sec on 1 B200 at M=10^6 (+ % of HBM roofline per firing)"
 UNIT = "firings/s"
 BYTES_PER_REACTION_FIRING = 32   # read T, P, a; write T
-# Measured once with `ncu --set full` (profiles/): dram bytes per launch of the bundle kernel at
-# the default workload; None until a capture exists for the shipped kernel.
-NCU_TRAFFIC_BYTES = {}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the bundle kernel, from the
+# `ncu --set full` capture of this command (profiles/r1_v4_bundle_kernel.md): 51.88 MB + 2.59 MB.
+# Far BELOW the algorithmic bytes: at M = 1e6 the (T,P,a) state lives in shared memory.
+NCU_TRAFFIC_BYTES = {"cfg4": 54471680}
 
 
 def parse_args():
@@ -262,6 +263,7 @@ def run_cuda(args):
                        else "independent trajectories", "l2": "flushed between steps (256 MB fill)",
                        "bundle_ctas": model.info("bundle_ctas"), "bundles": model.info("bundles"),
                        "block_threads": model.info("block_threads"),
+                       "state_in_shared_memory": bool(model.info("state_in_smem")),
                        "us_per_firing": 1e6 * kernel_s / firings},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},

@@ -97,11 +97,6 @@ struct BundleCtx {
   double p_val;
 };
 
-// Block-wide lexmin of the thread candidates, then all-gather of the S CTA partials through the
-// exchange slots (which is also the bundle barrier).  Every thread returns the bundle-wide
-// winner.  win.k == -2 signals a timeout.  fence = true additionally orders all earlier global
-// writes of every CTA before all later reads of every CTA (start and end of a trajectory; the
-// per-firing call does not need it).
 // Walker-warp state that outlives a firing: what it has prepared for this CTA's candidate.
 struct Spec {
   int pf_k;          // candidate whose walk data was last prefetched into L2
@@ -114,6 +109,9 @@ struct Spec {
   u64 seed, traj;
 };
 
+// Block-wide lexmin of the thread candidates, then all-gather of the S CTA partials through the
+// exchange slots (which is also the per-firing bundle barrier).  Every thread returns the
+// bundle-wide winner.  win.k == -2 signals a timeout.
 template <int BLOCK>
 __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<BLOCK> &ctx,
                                               u64 *exch, const uint32_t *nfire, int r,
