@@ -128,11 +128,41 @@ def test_cfg4_scaled(rt):
     _check_run(rt, net, x0, par["seed"], 0, 2000, math.inf, 2000)
 
 
-def test_cfg4_full_prefix(rt):
-    """BASELINE config 4 (M=1e6, the bench workload) in the bench launch shape: the oracle
-    does 300 firings (3e8 reaction-steps) in seconds; compare that prefix bit-exactly."""
+def test_cfg4_full_first_1e4(rt):
+    """BASELINE config 4 (M=1e6, the bench workload) in the launch shape bench.py times:
+    the first 1e4 firings, fired sequence and counts bit-exact, times to 1e-12 (the oracle
+    needs about a minute for its 1e10 reaction-steps)."""
     net, x0, par = W.make_config("cfg4")
-    _check_run(rt, net, x0, par["seed"], 0, 300, math.inf, 300)
+    g, o = _check_run(rt, net, x0, par["seed"], 0, 10_000, math.inf, 10_000)
+    assert g["firings"] == 10_000
+
+
+def test_cfg5a_full_size_prefix(rt):
+    """BASELINE config 5a (M=1e7: state streamed from global memory) at full size; the oracle
+    does 20 firings (2e8 reaction-steps) in seconds."""
+    net, x0, par = W.make_config("cfg5a")
+    with rt.Model(net) as m:
+        g = m.run(x0, par["seed"], 0, 20, math.inf, 20, want_state=True)
+        assert m.info("state_in_smem") == 0
+    o = _oracle().run(net, x0, par["seed"], 0, 20, math.inf, 20)
+    np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_allclose(g["trace_t"], o["trace_t"], rtol=RTOL_T, atol=0)
+    np.testing.assert_allclose(g["T"], o["T"], rtol=1e-10, atol=1e-12)
+
+
+def test_cfg5b_full_size_ensemble_prefix(rt):
+    """BASELINE config 5b: 64 trajectories of the M=1e5 network in the bench launch shape
+    (several bundles with on-chip state); every row against the oracle for 250 firings."""
+    net, x0, par = W.make_config("cfg5b")
+    n = 64
+    o = _oracle().ensemble(net, x0, par["seed"], 0, n, 250, math.inf, n_threads=8)
+    with rt.Model(net) as m:
+        g = m.ensemble(x0, par["seed"], 0, n, 250, math.inf)
+        assert m.info("ensemble_path") == 2 and m.info("state_in_smem") == 1
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["firings"], o["firings"])
+    np.testing.assert_allclose(g["t"], o["t"], rtol=RTOL_T)
 
 
 def test_t_end_stop_and_absorption(rt):
@@ -202,3 +232,59 @@ def test_prefix_property(rt):
         b = m.run(x0, 7, 0, 1200, trace_cap=1200)
     np.testing.assert_array_equal(a["trace_mu"], b["trace_mu"][:500])
     np.testing.assert_array_equal(a["trace_t"], b["trace_t"][:500])
+
+
+# ------------------------------------------------------------------ beyond the bit-exact horizon
+def _ks_and_moments(a, b):
+    from scipy import stats
+    p = stats.ks_2samp(a, b).pvalue
+    se = math.sqrt(a.var(ddof=1) / len(a) + b.var(ddof=1) / len(b))
+    return p, abs(a.mean() - b.mean()) / max(se, 1e-300)
+
+
+def test_cfg1_ensemble_statistics(rt):
+    """BASELINE config 1 in full: 1000 birth-death trajectories to t_end = 1000 (~2e4 firings each,
+    far past the bit-exact horizon).  Same Philox seed: rows identical to the oracle's.  A different
+    seed on the GPU side (so the test is not vacuous): mean and variance of X within 3 standard
+    errors of the stationary Poisson(100) law and of the oracle's sample, KS p > 0.01."""
+    from scipy import stats
+    net, x0, par = W.make_config("cfg1")
+    n = 1000
+    o = _oracle().ensemble(net, x0, par["seed"], 0, n, par["max_firings"], 1000.0, n_threads=8)
+    with rt.Model(net) as m:
+        same = m.ensemble(x0, par["seed"], 0, n, par["max_firings"], 1000.0)
+        other = m.ensemble(x0, par["seed"] + 12345, 0, n, par["max_firings"], 1000.0)
+    np.testing.assert_array_equal(same["x"], o["x"])
+    np.testing.assert_array_equal(same["firings"], o["firings"])
+    assert (other["stop"] == rt.RT_STOP_T_END).all() and (other["t"] == 1000.0).all()
+    xg, xo = other["x"][:, 0].astype(float), o["x"][:, 0].astype(float)
+    assert abs(xg.mean() - 100.0) < 3 * math.sqrt(100.0 / n)
+    assert abs(xg.var(ddof=1) - 100.0) < 3 * 100.0 * math.sqrt(2.0 / (n - 1)) + 3 * math.sqrt(100.0 / n)
+    p, z = _ks_and_moments(xg, xo)
+    assert p > 0.01 and z < 3.0
+    # exact law: KS against the Poisson(100) CDF is conservative for a discrete law
+    assert stats.kstest(xg, stats.poisson(100).cdf).pvalue > 0.01
+
+
+def test_cfg2_ensemble_statistics(rt):
+    """BASELINE config 2 shape (Lotka-Volterra, one thread per trajectory), t_end = 1 (~3e4 firings
+    per trajectory): same seed -> identical rows; different seed -> both species' marginals agree
+    with the oracle's (means within 3 SE, KS p > 0.01, Holm over the two species)."""
+    net, x0, par = W.make_config("cfg2")
+    n = 400
+    o = _oracle().ensemble(net, x0, par["seed"], 0, n, par["max_firings"], 1.0, n_threads=8)
+    with rt.Model(net) as m:
+        same = m.ensemble(x0, par["seed"], 0, n, par["max_firings"], 1.0)
+        other = m.ensemble(x0, par["seed"] + 777, 0, n, par["max_firings"], 1.0)
+        assert m.info("ensemble_path") == 1
+    np.testing.assert_array_equal(same["x"], o["x"])
+    np.testing.assert_array_equal(same["firings"], o["firings"])
+    ps = []
+    for j in range(2):
+        p, z = _ks_and_moments(other["x"][:, j].astype(float), o["x"][:, j].astype(float))
+        assert z < 3.0
+        ps.append(p)
+    ps.sort()
+    assert ps[0] > 0.01 / 2 and ps[1] > 0.01      # Holm-corrected
+    fz = _ks_and_moments(other["firings"].astype(float), o["firings"].astype(float))[1]
+    assert fz < 3.0
