@@ -292,6 +292,74 @@ __device__ __forceinline__ Cand scan_filtered(int tid, int k0, int cnt_pad, doub
   return best;
 }
 
+// The same filter over state streamed from global memory (HBM regime, cfg5a): 4 pairs of
+// reactions per thread and iteration, i.e. twelve 16-byte loads (192 B) in flight per thread
+// before any is used, and ~1/3 of the instructions of dividing everything, so that the pass is
+// bound by the memory system and not by issue slots.  Padding reactions (k >= M) hold a = 0.
+template <int NT, bool UPDATE>
+__device__ __forceinline__ Cand scan_filtered_global(int tid, int k0, int k1, double *T, double *P,
+                                                     double *A, double dprev, bool any_odd, bool &defer) {
+  constexpr int U = 4;
+  const float FINF = __int_as_float(0x7f800000);
+  double2 *T2 = reinterpret_cast<double2 *>(T);
+  const double2 *P2 = reinterpret_cast<const double2 *>(P);
+  const double2 *A2 = reinterpret_cast<const double2 *>(A);
+  const int q0 = k0 >> 1, q1 = k1 >> 1;
+  float m1 = FINF, m2 = FINF;
+  int i1 = k0;
+  for (int q = q0 + tid; q < q1; q += U * NT) {
+    double2 tt[U], pp[U], aa[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int qu = q + u * NT;
+      if (qu < q1) { tt[u] = __ldcg(T2 + qu); pp[u] = __ldcg(P2 + qu); aa[u] = __ldcg(A2 + qu); }
+      else { tt[u] = make_double2(0.0, 0.0); pp[u] = make_double2(1.0, 1.0); aa[u] = tt[u]; }  // q~ = +inf
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int qu = q + u * NT;
+      if (UPDATE) {
+        tt[u].x = __dadd_rn(tt[u].x, __dmul_rn(aa[u].x, dprev));
+        tt[u].y = __dadd_rn(tt[u].y, __dmul_rn(aa[u].y, dprev));
+        if (qu < q1) __stcg(T2 + qu, tt[u]);
+      }
+      float qf = __double2float_rn(__dmul_rn(__dsub_rn(pp[u].x, tt[u].x), rcp_approx(aa[u].x)));
+      m2 = fminf(m2, fmaxf(qf, m1));
+      if (qf < m1) { m1 = qf; i1 = 2 * qu; }
+      qf = __double2float_rn(__dmul_rn(__dsub_rn(pp[u].y, tt[u].y), rcp_approx(aa[u].y)));
+      m2 = fminf(m2, fmaxf(qf, m1));
+      if (qf < m1) { m1 = qf; i1 = 2 * qu + 1; }
+    }
+  }
+  Cand best;
+  best.dt = __longlong_as_double(0x7ff0000000000000ll);
+  best.k = 0x7fffffff;
+  const float thr = m1 * (1.0f + kFilterTol);
+  const bool decided = !any_odd && m1 >= 0x1.0p-100f && m1 <= 0x1.0p100f && m2 > thr;
+  if (decided) {
+    best.dt = waiting_time(__ldcg(P + i1), __ldcg(T + i1), __ldcg(A + i1));
+    best.k = i1;
+  } else if (UPDATE) {
+    defer = true;                               // left to the re-scan (see scan_filtered)
+  } else {
+    const bool all = any_odd || !(m1 >= 0x1.0p-100f && m1 <= 0x1.0p100f);
+    for (int q = q0 + tid; q < q1; q += NT) {
+      const double2 t2 = __ldcg(T2 + q), p2 = __ldcg(P2 + q), a2 = __ldcg(A2 + q);
+      float qf = __double2float_rn(__dmul_rn(__dsub_rn(p2.x, t2.x), rcp_approx(a2.x)));
+      if (all || qf <= thr) {
+        const double d = waiting_time(p2.x, t2.x, a2.x);
+        if (d < best.dt) { best.dt = d; best.k = 2 * q; }
+      }
+      qf = __double2float_rn(__dmul_rn(__dsub_rn(p2.y, t2.y), rcp_approx(a2.y)));
+      if (all || qf <= thr) {
+        const double d = waiting_time(p2.y, t2.y, a2.y);
+        if (d < best.dt) { best.dt = d; best.k = 2 * q + 1; }
+      }
+    }
+  }
+  return best;
+}
+
 // The per-firing pass of one thread over the reactions it owns.  UPDATE: also apply the
 // internal-time increment T_k += a_k * dprev (first pass); otherwise read-only (re-scan).
 // FULL: recompute a_k from X for every k (refresh_mode 1).
@@ -305,6 +373,7 @@ __device__ __forceinline__ Cand scan_own(const NetDev &net, const u64 *X, int ti
   best.dt = __longlong_as_double(0x7ff0000000000000ll);
   best.k = 0x7fffffff;
   if (SMEM && !full) return scan_filtered<NT, UPDATE>(tid, k0, cnt_pad, sT, sP, sA, dprev, any_odd, defer);
+  if (!SMEM && !full) return scan_filtered_global<NT, UPDATE>(tid, k0, k1, T, P, A, dprev, any_odd, defer);
   if (SMEM) {
     const int cnt = k1 - k0;
 #pragma unroll 4
@@ -712,7 +781,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         for (int i = tid; i < n; i += BLOCK) {
           const int k = list_k[i];
           if (SMEM) sA[k - k0] = list_a[i]; else __stcg(A + k, list_a[i]);
-          if (SMEM && filter_unsafe(list_a[i])) ctx.any_odd = 1;
+          if (filter_unsafe(list_a[i])) ctx.any_odd = 1;
           dirty[owner_thread<NT, SMEM>(k, k0)] = 1;
         }
         if (tid == 0 && ctx.p_k >= 0) {
