@@ -93,6 +93,7 @@ struct BundleCtx {
   int list_n;             // staged refreshes of this round
   int more;               // walker has entries left for another round
   int any_odd;            // some a_k of this CTA is outside the filter's safe range (sticky)
+  int n_stale;            // global-memory state: threads whose candidate must be re-scanned
   int p_k;                // reaction whose P was redrawn (or -1), and its new value
   double p_val;
 };
@@ -574,6 +575,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   __shared__ int4 list_d[kListCap];
   __shared__ double list_a[kListCap];
   __shared__ unsigned char dirty[BLOCK];
+  __shared__ int mybest_k[BLOCK];                    // reaction each stream thread proposes (-3: undecided)
+  __shared__ Cand redo[SMEM ? 1 : BLOCK];            // global-memory state: cooperative re-scan results
+  __shared__ short stale_list[SMEM ? 1 : BLOCK];
   extern __shared__ __align__(16) unsigned char dyn_smem[];
   PT_DECL
   const NetDev &net = p.net;
@@ -652,7 +656,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       uint32_t w_e0 = 0;
       bool w_csr = false;
       Cand best = none;
+      Cand extra = none;        // fresh waiting times of refreshed reactions this thread stored
 
+      if (is_walker && lane == 0) ctx.p_k = -1;   // (re)set below by the owner of the fired reaction
       if (is_walker && mu_prev >= 0) {
         // ===== walker warp: discrete updates of the previous firing (a-6, a-7, a-8) =====
         const bool owner = (mu_prev >= k0 && mu_prev < k1);
@@ -765,6 +771,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           bool defer = false;
           best = scan_own<NT, SMEM, true>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, dprev, full, cnt_pad,
                                           ctx.any_odd != 0, defer);
+          mybest_k[tid] = defer ? -3 : best.k;
           if (defer) dirty[tid] = 1;
         }
         PT_MARK(1)
@@ -778,29 +785,74 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
 #if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING == 1
         if (tid == 0 && gen < 512 && first_round) g_dbg[((size_t)r * 512 + gen) * 8 + 2] = (unsigned long long)n;
 #endif
+        // A refreshed reaction invalidates its owner's proposal only if it IS that proposal (the
+        // proposal is the minimum over the owner's other, unchanged reactions as well).  Then the
+        // owner re-scans; otherwise the new waiting time simply joins the reduction as one more
+        // candidate.  The reaction that fired (new P) always sends its owner to the re-scan.
+        const int pk_now = ctx.p_k;
         for (int i = tid; i < n; i += BLOCK) {
           const int k = list_k[i];
-          if (SMEM) sA[k - k0] = list_a[i]; else __stcg(A + k, list_a[i]);
-          if (filter_unsafe(list_a[i])) ctx.any_odd = 1;
-          dirty[owner_thread<NT, SMEM>(k, k0)] = 1;
+          const double a_new = list_a[i];
+          if (SMEM) sA[k - k0] = a_new; else __stcg(A + k, a_new);
+          if (filter_unsafe(a_new)) ctx.any_odd = 1;
+          const int o = owner_thread<NT, SMEM>(k, k0);
+          if (mybest_k[o] == k || mybest_k[o] == -3 || k == pk_now) {
+            dirty[o] = 1;
+          } else {
+            const double d = waiting_time(SMEM ? sP[k - k0] : __ldcg(P + k),
+                                          SMEM ? sT[k - k0] : __ldcg(T + k), a_new);
+            if (cand_less(d, k, extra)) { extra.dt = d; extra.k = k; }
+          }
         }
-        if (tid == 0 && ctx.p_k >= 0) {
-          const int k = ctx.p_k;
-          if (SMEM) sP[k - k0] = ctx.p_val; else __stcg(P + k, ctx.p_val);
-          dirty[owner_thread<NT, SMEM>(k, k0)] = 1;
-          ctx.p_k = -1;
+        if (tid == 0) {
+          if (first_round && pk_now >= 0) {
+            if (SMEM) sP[pk_now - k0] = ctx.p_val; else __stcg(P + pk_now, ctx.p_val);
+            dirty[owner_thread<NT, SMEM>(pk_now, k0)] = 1;
+          }
+          ctx.n_stale = 0;
         }
         __syncthreads();
         if (!more) break;
         first_round = false;
       }
       PT_MARK(2)
-      if (!is_walker && dirty[tid]) {            // re-scan (read-only) with the new a_k, P_mu
-        dirty[tid] = 0;
-        bool defer = false;
-        best = scan_own<NT, SMEM, false>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, 0.0, false, cnt_pad,
-                                         ctx.any_odd != 0, defer);
+      if (SMEM) {
+        if (!is_walker && dirty[tid]) {          // re-scan (read-only) with the new a_k, P_mu
+          dirty[tid] = 0;
+          bool defer = false;
+          best = scan_own<NT, SMEM, false>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, 0.0, false, cnt_pad,
+                                           ctx.any_odd != 0, defer);
+        }
+      } else {
+        // State in global memory: one thread re-reading its ~130 strided reactions is a chain of
+        // DRAM latencies (17 us on cfg5a).  The whole CTA shares the work instead: each warp takes
+        // one stale thread's reactions, 32 pairs at a time.
+        const bool was_stale = !is_walker && dirty[tid];
+        if (was_stale) { dirty[tid] = 0; stale_list[atomicAdd(&ctx.n_stale, 1)] = (short)tid; }
+        __syncthreads();
+        const int n_stale = ctx.n_stale;
+        if (n_stale > 0) {
+          const double2 *T2 = reinterpret_cast<const double2 *>(T);
+          const double2 *P2 = reinterpret_cast<const double2 *>(P);
+          const double2 *A2 = reinterpret_cast<const double2 *>(A);
+          for (int sidx = tid >> 5; sidx < n_stale; sidx += BLOCK / 32) {
+            const int d = stale_list[sidx];
+            Cand c = none;
+            for (int q = (k0 >> 1) + d + lane * NT; q < (k1 >> 1); q += 32 * NT) {
+              const double2 t2 = __ldcg(T2 + q), p2 = __ldcg(P2 + q), a2 = __ldcg(A2 + q);
+              double w = waiting_time(p2.x, t2.x, a2.x);
+              if (cand_less(w, 2 * q, c)) { c.dt = w; c.k = 2 * q; }
+              w = waiting_time(p2.y, t2.y, a2.y);
+              if (cand_less(w, 2 * q + 1, c)) { c.dt = w; c.k = 2 * q + 1; }
+            }
+            c = warp_lexmin(c);
+            if (lane == 0) redo[d] = c;
+          }
+          __syncthreads();
+          if (was_stale) best = redo[tid];
+        }
       }
+      if (cand_less(extra.dt, extra.k, best)) best = extra;
       if (ctx.abort_local) { status = RT_ERR_OVERFLOW; stop = 0; break; }
       if (finishing) break;
 
