@@ -72,7 +72,7 @@ struct rt_model {
   // staging for the host-pointer API
   DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t;
   // options
-  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0, opt_prefetch = 3;
+  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0, opt_prefetch = 7;
   // info
   int64_t kernel_launches = 0;
   int last_S = 0, last_B = 0, last_path = 0, last_state_smem = 0;
@@ -534,7 +534,7 @@ int rt_set_option(rt_model *m, const char *name, int64_t value) {
     if (value < 0 || value > 2) return RT_ERR_BAD_ARG;
     m->opt_ensemble_path = (int)value;
   } else if (!strcmp(name, "prefetch")) {
-    if (value < 0 || value > 3) return RT_ERR_BAD_ARG;
+    if (value < 0 || value > 7) return RT_ERR_BAD_ARG;
     m->opt_prefetch = (int)value;
   } else if (!strcmp(name, "x_replicas")) {
     if (value < 0 || value > 64) return RT_ERR_BAD_ARG;

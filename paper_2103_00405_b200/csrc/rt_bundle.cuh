@@ -31,7 +31,7 @@
 
 namespace rt {
 
-constexpr int kListCap = 512;       // refreshed reactions a CTA stages per round
+constexpr int kListCap = 256;       // refreshed reactions a CTA stages per round
 constexpr int kWalkerWarps = 1;
 constexpr int kMaxBundleCtas = 160; // CTAs that may share one trajectory (5 exchange slots per lane)
 constexpr int kSlotStride = 32;     // u64 words between exchange slots: 256 B, so the 148 slots that every
@@ -89,6 +89,7 @@ template <int BLOCK>
 struct BundleCtx {
   Cand warp_part[BLOCK / 32];
   Cand win;
+  int second_k;           // runner-up of the exchange (reaction index, or 0x7fffffff)
   int abort_local;        // a count left [0, xmax] (identical in every CTA: all replicate X)
   int list_n;             // staged refreshes of this round
   int more;               // walker has entries left for another round
@@ -97,122 +98,6 @@ struct BundleCtx {
   int p_k;                // reaction whose P was redrawn (or -1), and its new value
   double p_val;
 };
-
-// Walker-warp state that outlives a firing: what it has prepared for this CTA's candidate.
-struct Spec {
-  int pf_k;          // candidate whose walk data was last prefetched into L2
-  int k;             // candidate whose redraw is precomputed (lane 0), or -1
-  uint32_t n;        //   its new firing count
-  double P;          //   its new internal firing time P_k + E(seed, traj, k, n)
-  const double *sP;  // shared-memory P (nullptr: state in global memory)
-  const double *P_glob;
-  int k0;
-  u64 seed, traj;
-};
-
-// Block-wide lexmin of the thread candidates, then all-gather of the S CTA partials through the
-// exchange slots (which is also the per-firing bundle barrier).  Every thread returns the
-// bundle-wide winner.  win.k == -2 signals a timeout.
-template <int BLOCK>
-__device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<BLOCK> &ctx,
-                                              u64 *exch, const uint32_t *nfire, int r,
-                                              uint32_t &gen, Cand mine, bool fence, Spec &spec) {
-  constexpr int NT = BLOCK - 32 * kWalkerWarps;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  mine = warp_lexmin(mine);
-  if (lane == 0) ctx.warp_part[warp] = mine;
-  if (fence) __threadfence();
-  __syncthreads();
-  if (warp == 0) {
-    Cand c = ctx.warp_part[lane];                 // BLOCK / 32 <= 32 partials
-    if (lane >= BLOCK / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
-    c = warp_lexmin(c);
-    if (p.S > 1) {
-      const uint32_t tag = gen + 1u;
-      const u64 par = (u64)(((gen >> 1) & 1u) ^ 1u) << 63;     // never matches zeroed memory
-      u64 *buf = exch + (size_t)(gen & 1u) * (size_t)p.S * kSlotStride;
-#ifdef RT_PHASE_TIMING
-      if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 0] = gtime();
-#endif
-      if (lane == 0)
-        st_relaxed_v2(buf + (size_t)kSlotStride * r, (u64)__double_as_longlong(c.dt) | par,
-                      ((u64)tag << 32) | (u64)(uint32_t)c.k);
-      c.dt = __longlong_as_double(0x7ff0000000000000ll);
-      c.k = 0x7fffffff;
-      const long long t0 = clock64();
-      // Lane l gathers slots l, l+32, ...: all of its loads are in flight together, so the
-      // all-gather completes one L2 round trip after the last CTA has posted.
-      constexpr int kMaxPer = kMaxBundleCtas / 32;
-      unsigned pending = 0;
-      for (int i = 0; i < kMaxPer; ++i) if (lane + 32 * i < p.S) pending |= 1u << i;
-      while (pending) {
-        u64 w0[kMaxPer], w1[kMaxPer];
-#pragma unroll
-        for (int i = 0; i < kMaxPer; ++i)
-          if (pending & (1u << i)) ld_relaxed_v2(buf + (size_t)kSlotStride * (lane + 32 * i), w0[i], w1[i]);
-#pragma unroll
-        for (int i = 0; i < kMaxPer; ++i)
-          if ((pending & (1u << i)) && (uint32_t)(w1[i] >> 32) == tag && (w0[i] >> 63) == (par >> 63)) {
-            pending &= ~(1u << i);
-            const double dt = __longlong_as_double((long long)(w0[i] & 0x7fffffffffffffffull));
-            const int k = (int)(uint32_t)(w1[i] & 0x7fffffffu);
-            if (cand_less(dt, k, c)) { c.dt = dt; c.k = k; }
-          }
-        if (pending && clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); c.k = -2; break; }
-      }
-      const bool timed_out = __any_sync(0xffffffffu, c.k == -2);
-#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING >= 2
-      if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 1] = gtime();
-#endif
-      c = warp_lexmin(c);
-      if (timed_out) c.k = -2;
-    }
-    if (lane == 0) ctx.win = c;
-  } else if (warp == BLOCK / 32 - 1 && !fence) {
-    // Walker warp, idle during the exchange.  If this CTA's candidate wins (it usually stays the
-    // candidate for many firings before it does), this CTA must redraw P_k (Philox + log, the
-    // longest serial piece of a firing) and every CTA will need the candidate's stoich row and
-    // the dependency entries of its species, all DRAM-cold (each reaction fires rarely).
-    // Do the redraw now, speculatively, and pull the rest into L2 -- once per candidate.
-    Cand c = ctx.warp_part[lane];
-    if (lane >= BLOCK / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
-    c = warp_lexmin(c);
-    if (c.k < p.net.M && c.k != spec.k && lane == 0 && (p.prefetch & 2)) {
-      const uint32_t n1 = nfire[c.k] + 1u;
-      const double pold = spec.sP ? spec.sP[c.k - spec.k0] : __ldcg(spec.P_glob + c.k);
-      spec.P = __dadd_rn(pold, exp_draw(spec.seed, spec.traj, (uint32_t)c.k, n1));
-      spec.n = n1;
-      spec.k = c.k;
-    }
-    if (c.k != spec.pf_k && c.k < p.net.M && (p.prefetch & 1)) {
-      spec.pf_k = c.k;
-      int4 ent = make_int4(-1, 0, 0, 0);
-      if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(p.net.srow) + (size_t)c.k * 4 + lane);
-#pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const int j = __shfl_sync(0xffffffffu, ent.x, e);
-        const uint32_t lo = (uint32_t)__shfl_sync(0xffffffffu, ent.z, e);
-        const uint32_t hi = (uint32_t)__shfl_sync(0xffffffffu, ent.w, e);
-        if (j >= 0 && hi != 0xffffffffu)            // hubs stay hot by themselves
-          for (uint32_t i = lo + 4u * lane; i < hi; i += 128u)
-            prefetch_l2(reinterpret_cast<const char *>(p.net.dep) + (size_t)i * 32);
-      }
-    }
-  }
-  gen += 1u;
-  if (fence) {
-    __syncthreads();
-    __threadfence();
-  } else {
-    // The stream warps leave as soon as warp 0 has the winner; the walker warp, which may still
-    // be busy with its speculative work, pairs with warp 0 on a barrier of its own.
-    if (warp == 0) asm volatile("bar.arrive 2, 64;" ::: "memory");
-    if (warp == BLOCK / 32 - 1) asm volatile("bar.sync 2, 64;" ::: "memory");
-    else asm volatile("bar.sync 1, %0;" ::"r"(NT) : "memory");
-  }
-  return ctx.win;
-}
-
 
 // ---- filtered scan (state in shared memory) ----------------------------------------------------
 // The argmin needs the correctly rounded quotient of only ONE of a thread's reactions: the others
@@ -535,6 +420,160 @@ __device__ __forceinline__ long long x_peek(const u64 *Xv, int j, int v, u64 ver
   return (x < 0 || x > xmax) ? -1 : x;
 }
 
+// Walker-warp state that outlives a firing: what it has prepared for this CTA's candidate.
+struct Spec {
+  int pf_k;          // candidate whose walk data was last prefetched into L2
+  int k;             // candidate whose redraw is precomputed (lane 0), or -1
+  uint32_t n;        //   its new firing count
+  double P;          //   its new internal firing time P_k + E(seed, traj, k, n)
+  const double *sP;  // shared-memory P (nullptr: state in global memory)
+  const double *P_glob;
+  int k0, k1;
+  u64 seed, traj;
+  // pre-walk: the dependency entries of reaction pw_k that fall in [k0, k1), compacted in shared
+  // memory (pw_d, pw_c) ahead of time; pw_ent = its stoich row (lanes 0..3).  Network data only,
+  // so it stays valid until another reaction is pre-walked.
+  int k2;            // runner-up of the last exchange: the likeliest next winner
+  int pw_k, pw_n;
+  int4 pw_ent;
+  int4 *pw_d;
+  double *pw_c;
+};
+
+// Block-wide lexmin of the thread candidates, then all-gather of the S CTA partials through the
+// exchange slots (which is also the per-firing bundle barrier).  Every thread returns the
+// bundle-wide winner.  win.k == -2 signals a timeout.
+template <int BLOCK>
+__device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<BLOCK> &ctx,
+                                              u64 *exch, const uint32_t *nfire, int r,
+                                              uint32_t &gen, Cand mine, bool fence, Spec &spec) {
+  constexpr int NT = BLOCK - 32 * kWalkerWarps;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  mine = warp_lexmin(mine);
+  if (lane == 0) ctx.warp_part[warp] = mine;
+  if (fence) __threadfence();
+  __syncthreads();
+  if (warp == 0) {
+    Cand c = ctx.warp_part[lane];                 // BLOCK / 32 <= 32 partials
+    if (lane >= BLOCK / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
+    c = warp_lexmin(c);
+    Cand c2;                                      // this lane's second-best slot (runner-up search)
+    c2.dt = __longlong_as_double(0x7ff0000000000000ll); c2.k = 0x7fffffff;
+    if (p.S > 1) {
+      const uint32_t tag = gen + 1u;
+      const u64 par = (u64)(((gen >> 1) & 1u) ^ 1u) << 63;     // never matches zeroed memory
+      u64 *buf = exch + (size_t)(gen & 1u) * (size_t)p.S * kSlotStride;
+#ifdef RT_PHASE_TIMING
+      if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 0] = gtime();
+#endif
+      if (lane == 0)
+        st_relaxed_v2(buf + (size_t)kSlotStride * r, (u64)__double_as_longlong(c.dt) | par,
+                      ((u64)tag << 32) | (u64)(uint32_t)c.k);
+      c.dt = __longlong_as_double(0x7ff0000000000000ll);
+      c.k = 0x7fffffff;
+      const long long t0 = clock64();
+      // Lane l gathers slots l, l+32, ...: all of its loads are in flight together, so the
+      // all-gather completes one L2 round trip after the last CTA has posted.
+      constexpr int kMaxPer = kMaxBundleCtas / 32;
+      unsigned pending = 0;
+      for (int i = 0; i < kMaxPer; ++i) if (lane + 32 * i < p.S) pending |= 1u << i;
+      while (pending) {
+        u64 w0[kMaxPer], w1[kMaxPer];
+#pragma unroll
+        for (int i = 0; i < kMaxPer; ++i)
+          if (pending & (1u << i)) ld_relaxed_v2(buf + (size_t)kSlotStride * (lane + 32 * i), w0[i], w1[i]);
+#pragma unroll
+        for (int i = 0; i < kMaxPer; ++i)
+          if ((pending & (1u << i)) && (uint32_t)(w1[i] >> 32) == tag && (w0[i] >> 63) == (par >> 63)) {
+            pending &= ~(1u << i);
+            const double dt = __longlong_as_double((long long)(w0[i] & 0x7fffffffffffffffull));
+            const int k = (int)(uint32_t)(w1[i] & 0x7fffffffu);
+            if (cand_less(dt, k, c)) { c2 = c; c.dt = dt; c.k = k; }
+            else if (cand_less(dt, k, c2)) { c2.dt = dt; c2.k = k; }
+          }
+        if (pending && clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); c.k = -2; break; }
+      }
+      const bool timed_out = __any_sync(0xffffffffu, c.k == -2);
+#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING >= 2
+      if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 1] = gtime();
+#endif
+      const Cand mine_best = c;
+      c = warp_lexmin(c);
+      // runner-up = best of everything but the winner: the likeliest winner of the next firing
+      c2 = warp_lexmin((mine_best.k == c.k) ? c2 : mine_best);
+      if (timed_out) c.k = -2;
+    }
+    if (lane == 0) { ctx.win = c; ctx.second_k = (c2.dt < __longlong_as_double(0x7ff0000000000000ll)) ? c2.k : 0x7fffffff; }
+  } else if (warp == BLOCK / 32 - 1 && !fence) {
+    // Walker warp, idle during the exchange.  If this CTA's candidate wins (it usually stays the
+    // candidate for many firings before it does), this CTA must redraw P_k (Philox + log, the
+    // longest serial piece of a firing) and every CTA will need the candidate's stoich row and
+    // the dependency entries of its species, all DRAM-cold (each reaction fires rarely).
+    // Do the redraw now, speculatively, and pull the rest into L2 -- once per candidate.
+    Cand c = ctx.warp_part[lane];
+    if (lane >= BLOCK / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
+    c = warp_lexmin(c);
+    if ((p.prefetch & 4) && spec.k2 != spec.pw_k && spec.k2 < p.net.M && spec.k1 > spec.k0) {
+      // pre-walk of the runner-up: row -> ranges -> this CTA's dependency entries, into pw_d / pw_c
+      const int k2 = spec.k2;
+      int4 ent = make_int4(-1, 0, 0, 0);
+      if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(p.net.srow) + (size_t)k2 * 4 + lane);
+      spec.pw_k = -1;
+      if (__shfl_sync(0xffffffffu, ent.x, 0) != -2) {
+        uint32_t lo = 0, hi = 0;
+        if (ent.x >= 0) { lo = (uint32_t)ent.z; hi = (uint32_t)ent.w; narrow_range(p.net, lo, hi, spec.k0, spec.k1); }
+        Ranges rg;
+        uint32_t acc = 0;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          rg.lo[e] = __shfl_sync(0xffffffffu, lo, e);
+          acc += __shfl_sync(0xffffffffu, hi - lo, e);
+          rg.end[e] = acc;
+        }
+        uint32_t f = 0;
+        int n = 0;
+        if (!walk_scan(p.net, rg, f, spec.k0, spec.k1, lane, n, spec.pw_d, spec.pw_c)) {
+          spec.pw_k = k2; spec.pw_n = n; spec.pw_ent = ent;
+        }
+      }
+    }
+    if (c.k < p.net.M && c.k != spec.k && lane == 0 && (p.prefetch & 2)) {
+      const uint32_t n1 = nfire[c.k] + 1u;
+      const double pold = spec.sP ? spec.sP[c.k - spec.k0] : __ldcg(spec.P_glob + c.k);
+      spec.P = __dadd_rn(pold, exp_draw(spec.seed, spec.traj, (uint32_t)c.k, n1));
+      spec.n = n1;
+      spec.k = c.k;
+    }
+    if (c.k != spec.pf_k && c.k < p.net.M && (p.prefetch & 1)) {
+      spec.pf_k = c.k;
+      int4 ent = make_int4(-1, 0, 0, 0);
+      if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(p.net.srow) + (size_t)c.k * 4 + lane);
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int j = __shfl_sync(0xffffffffu, ent.x, e);
+        const uint32_t lo = (uint32_t)__shfl_sync(0xffffffffu, ent.z, e);
+        const uint32_t hi = (uint32_t)__shfl_sync(0xffffffffu, ent.w, e);
+        if (j >= 0 && hi != 0xffffffffu)            // hubs stay hot by themselves
+          for (uint32_t i = lo + 4u * lane; i < hi; i += 128u)
+            prefetch_l2(reinterpret_cast<const char *>(p.net.dep) + (size_t)i * 32);
+      }
+    }
+  }
+  gen += 1u;
+  if (fence) {
+    __syncthreads();
+    __threadfence();
+  } else {
+    // The stream warps leave as soon as warp 0 has the winner; the walker warp, which may still
+    // be busy with its speculative work, pairs with warp 0 on a barrier of its own.
+    if (warp == 0) asm volatile("bar.arrive 2, 64;" ::: "memory");
+    if (warp == BLOCK / 32 - 1) { asm volatile("bar.sync 2, 64;" ::: "memory"); spec.k2 = ctx.second_k; }
+    else asm volatile("bar.sync 1, %0;" ::"r"(NT) : "memory");
+  }
+  return ctx.win;
+}
+
+
 // Fenced barrier over the CTAs of a bundle (start and end of a trajectory): all earlier global
 // writes of every CTA are visible to all later reads of every CTA.  Uses the exchange slots and
 // generation counter of bundle_argmin.  Returns false on a timeout.
@@ -573,6 +612,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   __shared__ BundleCtx<BLOCK> ctx;
   __shared__ int list_k[kListCap];
   __shared__ int4 list_d[kListCap];
+  __shared__ int4 pw_d[kListCap];
+  __shared__ double pw_c[kListCap];
   __shared__ double list_a[kListCap];
   __shared__ unsigned char dirty[BLOCK];
   __shared__ int mybest_k[BLOCK];                    // reaction each stream thread proposes (-3: undecided)
@@ -607,6 +648,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   uint32_t gen = 0;   // exchange generation, identical in every CTA of the bundle
   Spec spec;
   spec.pf_k = -1; spec.k = -1; spec.n = 0u; spec.P = 0.0;
+  spec.k2 = 0x7fffffff; spec.pw_k = -1; spec.pw_n = 0; spec.pw_ent = make_int4(-1, 0, 0, 0);
+  spec.pw_d = pw_d; spec.pw_c = pw_c; spec.k1 = 0;
   spec.sP = nullptr; spec.P_glob = nullptr; spec.k0 = 0; spec.seed = p.seed; spec.traj = 0;
   dirty[tid] = 0;
   if (tid == 0) { ctx.abort_local = 0; ctx.list_n = 0; ctx.more = 0; ctx.p_k = -1; ctx.any_odd = 0; }
@@ -615,7 +658,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
 
   for (u64 it = (u64)b; it < p.n_traj; it += (u64)p.B) {
     const u64 traj = p.traj_first + it;
-    spec.k = -1; spec.traj = traj; spec.sP = SMEM ? sP : nullptr; spec.P_glob = P; spec.k0 = k0;
+    spec.k = -1; spec.traj = traj; spec.sP = SMEM ? sP : nullptr; spec.P_glob = P; spec.k0 = k0; spec.k1 = k1;
+    spec.k2 = 0x7fffffff;
     const bool tracing = (it == 0) && p.trace_cap > 0 && r == 0;
 
     // ---- a-0: X = x0 (slices, version 0), then T = 0, P = E(k,0), a = a(X0), n = 0 for the own range
@@ -655,6 +699,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       int w_e = 0, w_ne = 0;    // CSR rows (more than 4 changed species): species cursor / count
       uint32_t w_e0 = 0;
       bool w_csr = false;
+      int pre_n = -1;           // >= 0: the pre-walk hit, list_k / list_a already hold pre_n refreshes
       Cand best = none;
       Cand extra = none;        // fresh waiting times of refreshed reactions this thread stored
 
@@ -668,11 +713,57 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           c_old = nfire[mu_prev];
           p_old = SMEM ? sP[mu_prev - k0] : __ldcg(P + mu_prev);
         }
-        int4 ent = make_int4(-1, 0, 0, 0);      // lane e < 4: (j, v, lo, hi) of the e-th changed species
-        if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(net.srow) + (size_t)mu_prev * 4 + lane);
+        const bool hit = !full && spec.pw_k == mu_prev;      // pre-walked while the exchange ran
+        int4 ent = spec.pw_ent;                 // lane e < 4: (j, v, lo, hi) of the e-th changed species
+        if (!hit) {
+          ent = make_int4(-1, 0, 0, 0);
+          if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(net.srow) + (size_t)mu_prev * 4 + lane);
+        }
         w_csr = __shfl_sync(0xffffffffu, ent.x, 0) == -2;
         PT_G(4)
-        if (!w_csr) {
+        if (hit) {
+          // One L2 round trip: the X words of the changed species and of the reactants of the
+          // first 32 pre-walked entries are loaded together; a word that does not yet carry this
+          // firing's version is brought up to date locally (X_j + v_j).
+          const bool active = ent.x >= 0;
+          const bool has0 = lane < spec.pw_n;
+          int4 d0 = make_int4(0, 0, -1, 0);
+          double c0 = 0.0;
+          u64 w1 = 0, w2 = 0;
+          if (has0) {
+            d0 = pw_d[lane]; c0 = pw_c[lane];
+            w1 = __ldcg(X + d0.y);
+            w2 = __ldcg(X + (d0.z >= 0 ? d0.z : d0.y));
+          }
+          bool done = false;
+          long long xn = 0;
+          if (active) xn = x_peek(X, ent.x, ent.y, fired, net.xmax, done);
+          const bool bad = __any_sync(0xffffffffu, active && xn < 0);
+          if (bad) { if (lane == 0) ctx.abort_local = 1; }
+          else if (active && !done) atomicMax(X + ent.x, x_pack(fired, xn));
+          long long x1 = x_count(w1), x2 = x_count(w2);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int je = __shfl_sync(0xffffffffu, ent.x, e);
+            const long long ve = (long long)__shfl_sync(0xffffffffu, ent.y, e);
+            if (je == d0.y && x_version(w1) != fired) x1 += ve;
+            if (je == d0.z && x_version(w2) != fired) x2 += ve;
+          }
+          __syncwarp();
+          if (has0) {
+            double a = __dmul_rn(c0, __ll2double_rn(binom(x1, d0.w & 0xff)));
+            if (d0.z >= 0) a = __dmul_rn(a, __ll2double_rn(binom(x2, (d0.w >> 8) & 0xff)));
+            if (d0.w & 0x10000) a = propensity(net, X, d0.x);       // > 2 reactants: after the update
+            list_k[lane] = d0.x;
+            list_a[lane] = a;
+          }
+          for (int i = lane + 32; i < spec.pw_n; i += 32) {        // more than 32: plain path
+            const int4 d = pw_d[i];
+            list_k[i] = d.x;
+            list_a[i] = propensity_dep(net, X, d, pw_c[i]);
+          }
+          pre_n = spec.pw_n;
+        } else if (!w_csr) {
           // a-6: X += v_mu (Eq.5); nothing is written if any count would leave [0, xmax]
           const bool active = ent.x >= 0;
           bool done = false;
@@ -745,7 +836,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           // ===== walker warp: dependency walk (a-1 for k in D(mu) that fall in [k0, k1)) =====
           int n = 0;
           bool more = false;
-          if (!w_csr) {
+          if (pre_n >= 0) {
+            n = first_round ? pre_n : 0;
+          } else if (!w_csr) {
             more = walk_scan(net, rg, w_f, k0, k1, lane, n, list_d, list_a);
           } else {
             while (w_e < w_ne) {
@@ -764,7 +857,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
               w_f = 0;
             }
           }
-          walk_finish(net, X, lane, n, list_d, list_k, list_a);
+          if (pre_n < 0) walk_finish(net, X, lane, n, list_d, list_k, list_a);
           if (lane == 0) { ctx.list_n = n; ctx.more = more ? 1 : 0; }
         } else if (first_round) {
           // ===== stream warps: a-5 of the previous firing fused with a-2/a-3 of this one =====
