@@ -443,7 +443,7 @@ struct Spec {
 // Block-wide lexmin of the thread candidates, then all-gather of the S CTA partials through the
 // exchange slots (which is also the per-firing bundle barrier).  Every thread returns the
 // bundle-wide winner.  win.k == -2 signals a timeout.
-template <int BLOCK>
+template <int BLOCK, bool PREWALK>
 __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<BLOCK> &ctx,
                                               u64 *exch, const uint32_t *nfire, int r,
                                               uint32_t &gen, Cand mine, bool fence, Spec &spec) {
@@ -513,7 +513,7 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
     Cand c = ctx.warp_part[lane];
     if (lane >= BLOCK / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
     c = warp_lexmin(c);
-    if ((p.prefetch & 4) && spec.k2 != spec.pw_k && spec.k2 < p.net.M && spec.k1 > spec.k0) {
+    if (PREWALK && (p.prefetch & 4) && spec.k2 != spec.pw_k && spec.k2 < p.net.M && spec.k1 > spec.k0) {
       // pre-walk of the runner-up: row -> ranges -> this CTA's dependency entries, into pw_d / pw_c
       const int k2 = spec.k2;
       int4 ent = make_int4(-1, 0, 0, 0);
@@ -612,8 +612,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   __shared__ BundleCtx<BLOCK> ctx;
   __shared__ int list_k[kListCap];
   __shared__ int4 list_d[kListCap];
-  __shared__ int4 pw_d[kListCap];
-  __shared__ double pw_c[kListCap];
+  __shared__ int4 pw_d[SMEM ? kListCap : 1];
+  __shared__ double pw_c[SMEM ? kListCap : 1];
   __shared__ double list_a[kListCap];
   __shared__ unsigned char dirty[BLOCK];
   __shared__ int mybest_k[BLOCK];                    // reaction each stream thread proposes (-3: undecided)
@@ -713,7 +713,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           c_old = nfire[mu_prev];
           p_old = SMEM ? sP[mu_prev - k0] : __ldcg(P + mu_prev);
         }
-        const bool hit = !full && spec.pw_k == mu_prev;      // pre-walked while the exchange ran
+        const bool hit = SMEM && !full && spec.pw_k == mu_prev;   // (pre-walk: shared-memory state only)      // pre-walked while the exchange ran
         int4 ent = spec.pw_ent;                 // lane e < 4: (j, v, lo, hi) of the e-th changed species
         if (!hit) {
           ent = make_int4(-1, 0, 0, 0);
@@ -951,7 +951,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
 
       // ---- a-3 argmin over the bundle
       PT_MARK(3)
-      const Cand win = bundle_argmin<BLOCK>(p, ctx, exch, nfire, r, gen, best, false, spec);
+      const Cand win = bundle_argmin<BLOCK, SMEM>(p, ctx, exch, nfire, r, gen, best, false, spec);
       PT_MARK(4)
       if (win.k == -2) return;
 
