@@ -720,6 +720,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(net.srow) + (size_t)mu_prev * 4 + lane);
         }
         w_csr = __shfl_sync(0xffffffffu, ent.x, 0) == -2;
+#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING == 1
+        if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 3] = hit ? 1ull : 0ull;
+#endif
         PT_G(4)
         if (hit) {
           // One L2 round trip: the X words of the changed species and of the reactants of the
