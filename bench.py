@@ -32,9 +32,9 @@ METRIC = "reaction firings/sec on 1 B200 at M=10^6 (+ % of HBM roofline per firi
 UNIT = "firings/s"
 BYTES_PER_REACTION_FIRING = 32   # read T, P, a; write T
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the bundle kernel, from the
-# `ncu --set full` capture of this command (profiles/r1_v4_bundle_kernel.md): 51.88 MB + 2.59 MB.
+# `ncu --set full` capture of this command (profiles/r1_v5_bundle_kernel.md): 51.45 MB + 2.31 MB.
 # Far BELOW the algorithmic bytes: at M = 1e6 the (T,P,a) state lives in shared memory.
-NCU_TRAFFIC_BYTES = {"cfg4": 54471680}
+NCU_TRAFFIC_BYTES = {"cfg4": 53759744}
 
 
 def parse_args():
