@@ -138,6 +138,11 @@ int rt_sync(rt_model *m, void *stream);
  *   "bundle_ctas"    CTAs cooperating on one trajectory; 0 = choose automatically
  *   "ensemble_path"  0 = automatic, 1 = force one-thread-per-trajectory kernel,
  *                    2 = force the bundle (CTA-group-per-trajectory) kernel
+ *   "state_mode"     0 = keep (T,P,a) in shared memory when a CTA's share fits (default),
+ *                    1 = always stream it from global memory (the regime of M > ~1.1e6)
+ *   "prefetch"       bit 0: L2 prefetch of the candidate's walk data, bit 1: speculative redraw,
+ *                    bit 2: pre-walk of the exchange's runner-up (default 7 = all)
+ *   "x_replicas"     copies of X per trajectory the CTAs spread their updates over (default 1)
  * Returns RT_ERR_BAD_ARG for an unknown name or value. */
 int rt_set_option(rt_model *m, const char *name, int64_t value);
 
@@ -145,7 +150,8 @@ int rt_set_option(rt_model *m, const char *name, int64_t value);
  *   "kernel_launches"  kernels launched by this model so far
  *   "bundle_ctas", "bundles", "block_threads"  shape of the last bundle launch
  *   "ensemble_path"    path taken by the last rt_ensemble call (1 or 2)
- *   "num_sms", "dep_entries", "max_sigma"
+ *   "state_in_smem"    1 if the last bundle launch kept (T,P,a) in shared memory
+ *   "num_sms", "dep_entries", "max_sigma", "hub_species"
  * Unknown name: returns RT_ERR_BAD_ARG and leaves *value alone. */
 int rt_get_info(const rt_model *m, const char *name, int64_t *value);
 

@@ -5,7 +5,7 @@
 //
 // Every CTA owns a fixed contiguous range [k0, k1) of reactions.  Its (T, P, a) triples live
 //   * in SHARED MEMORY for the whole trajectory when the range fits (STATE_SMEM: M up to
-//     ~1.3e6 on 148 SMs) -- the per-firing pass then never leaves the SM;
+//     ~1.1e6 on 148 SMs) -- the per-firing pass then never leaves the SM;
 //   * in global memory otherwise (structure-of-arrays fp64, 16-byte vector accesses,
 //     24 B read + 8 B written per reaction per firing -- the HBM-streaming regime).
 //
@@ -21,8 +21,10 @@
 //                  entries (k, reactants, sigma, c_k) -> new a_k for the k in [k0, k1).
 // The stream uses the OLD a_k, which is exactly the propensity that held during the elapsed
 // interval, so T is right for every k; only the waiting times of the refreshed reactions (and
-// of mu) are stale.  After one CTA barrier the new a_k / P_mu are stored, the threads that own
-// a refreshed reaction re-scan their few reactions (read-only), and the block argmin follows.
+// of mu) are stale.  After one CTA barrier the new a_k / P_mu are stored; a refreshed reaction
+// joins the reduction as a fresh candidate, and only a thread whose own proposal was refreshed
+// (or fired) re-scans its reactions (read-only); the block argmin follows.  While the exchange
+// runs, the walker warp pre-walks the runner-up, the likeliest next winner (see Spec).
 // The CTA partials are combined by an all-gather through L2 (one 16-byte slot per CTA,
 // self-validating words, double-buffered), which doubles as the per-firing bundle barrier.
 #pragma once
