@@ -35,6 +35,12 @@ BYTES_PER_REACTION_FIRING = 32   # read T, P, a; write T (DESIGN.md "algorithmic
 # `ncu --set full` capture of this command (profiles/r1_v5_bundle_kernel.md): 51.45 MB + 2.31 MB.
 # Far BELOW the algorithmic bytes: at M = 1e6 the (T,P,a) state lives in shared memory.
 NCU_TRAFFIC_BYTES = {"cfg4": 53759744}
+# Small-network ensembles (cfg1, cfg2: one thread per trajectory, state in shared memory) are bound
+# by plain ALU issue, not memory.  Thread instructions per trajectory-step, from
+# `ncu --metrics smsp__thread_inst_executed.sum` over a whole launch:
+THREAD_INSTR_PER_STEP = {"cfg1": 382.0, "cfg2": 511.2}
+# issue peak: 148 SMs x 4 schedulers x 32 lanes x 1.965 GHz (B200_PROFILING.md unit counts / clocks)
+ALU_PEAK_GINSTR = 148 * 4 * 32 * 1.965
 
 
 def parse_args():
@@ -43,7 +49,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="cfg4", choices=["cfg3", "cfg4", "cfg5a", "cfg5b"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5a", "cfg5b"])
     ap.add_argument("--firings", type=int, default=0, help="firings per step (0 = the config's)")
     ap.add_argument("--scale", type=float, default=1.0, help="shrink N, M (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -160,6 +166,7 @@ def run_cuda(args):
     N, M = int(net["n_species"]), int(net["n_reactions"])
     firings = args.firings or par["max_firings"]
     n_traj = par["n_traj"]
+    t_end = float(par.get("t_end", math.inf)) if args.workload in ("cfg1", "cfg2") else math.inf
     seed = par["seed"]
     traj0 = rank * n_traj                       # replicas: every rank its own trajectory ids
     model = rt.Model(net, local)
@@ -177,10 +184,10 @@ def run_cuda(args):
 
     def step_dev():
         if n_traj == 1:
-            rc = rt.rt_run_dev(model.handle, x0_dev, seed, traj0, firings, math.inf, x_out_dev,
+            rc = rt.rt_run_dev(model.handle, x0_dev, seed, traj0, firings, t_end, x_out_dev,
                                res_dev, tmu_dev, tt_dev, trace_cap)
         else:
-            rc = rt.rt_ensemble_dev(model.handle, x0_dev, seed, traj0, n_traj, firings, math.inf,
+            rc = rt.rt_ensemble_dev(model.handle, x0_dev, seed, traj0, n_traj, firings, t_end,
                                     x_out_dev, res_dev)
         if rc != rt.RT_OK:
             raise rt.RtError(rc, "rt_run_dev")
@@ -197,7 +204,13 @@ def run_cuda(args):
     if rt.rt_sync(model.handle) != rt.RT_OK:
         raise SystemExit("bench.py: device reported an error during warm-up")
     done = res_dev.cpu().numpy().view(rt.RESULT_DTYPE)
-    assert (done["firings"] == firings).all() and (done["status"] == 0).all(), done
+    assert (done["status"] == 0).all(), done
+    if math.isinf(t_end):
+        assert (done["firings"] == firings).all(), done
+    else:
+        # (a Lotka-Volterra trajectory may also die out -> absorbed, or explode -> max_firings)
+        assert (done["stop"] >= rt.RT_STOP_T_END).all() and (done["stop"] == rt.RT_STOP_T_END).mean() > 0.9, done
+    fired_per_step = int(done["firings"].sum())      # trajectory-steps of one step (all trajectories)
 
     # ---- timed region: K steps, device-timed; per-step events bracket the kernel launch only
     # (L2 flush sits between steps, outside the per-step events but inside the barrier bracket).
@@ -219,7 +232,7 @@ def run_cuda(args):
     if world > 1:
         dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
     total_s = float(total_ms.item()) * 1e-3
-    units = firings * n_traj * args.steps * world
+    units = fired_per_step * args.steps * world
     value = units / total_s
 
     # ---- e2e: the host-pointer C-ABI call a user makes; copies inside the timed region
@@ -228,9 +241,9 @@ def run_cuda(args):
 
     def step_host():
         if n_traj == 1:
-            out = model.run(x0_pin, seed, traj0, firings, math.inf, trace_cap=e2e_tr)
+            out = model.run(x0_pin, seed, traj0, firings, t_end, trace_cap=e2e_tr)
             return out["firings"]
-        out = model.ensemble(x0_pin, seed, traj0, n_traj, firings, math.inf)
+        out = model.ensemble(x0_pin, seed, traj0, n_traj, firings, t_end)
         return int(out["firings"].sum())
 
     step_host()
@@ -250,7 +263,7 @@ def run_cuda(args):
     if rank == 0:
         peak, peak_src = peaks()
         kernel_s = (sum(step_ms) / len(step_ms)) * 1e-3          # one bundle-kernel launch per step
-        alg_bytes = BYTES_PER_REACTION_FIRING * M * firings * n_traj
+        alg_bytes = BYTES_PER_REACTION_FIRING * M * fired_per_step
         achieved = alg_bytes / kernel_s / 1e9
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -258,13 +271,14 @@ def run_cuda(args):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": args.workload, "n_species": N, "n_reactions": M,
-                       "trajectories_per_step": n_traj, "firings_per_step": firings * n_traj,
+                       "trajectories_per_step": n_traj, "firings_per_step": fired_per_step,
                        "parallelism": "replicas only (one trajectory per GPU)" if n_traj == 1
                        else "independent trajectories", "l2": "flushed between steps (256 MB fill)",
                        "bundle_ctas": model.info("bundle_ctas"), "bundles": model.info("bundles"),
                        "block_threads": model.info("block_threads"),
                        "state_in_shared_memory": bool(model.info("state_in_smem")),
-                       "us_per_firing": 1e6 * kernel_s / firings},
+                       "us_per_firing": 1e6 * kernel_s / fired_per_step * n_traj,
+                       "ensemble_path": model.info("ensemble_path")},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},
             "gpu_launches": int(launches),
@@ -275,12 +289,35 @@ def run_cuda(args):
                          "algorithmic_bytes_per_launch": alg_bytes,
                          "frac_of_8TBs_nominal": achieved / 8000.0},
         }
+        if args.workload in THREAD_INSTR_PER_STEP:
+            # one thread per trajectory, state in shared memory: plain ALU issue is the bound
+            ginstr = THREAD_INSTR_PER_STEP[args.workload] * fired_per_step / kernel_s / 1e9
+            line["roofline"] = {"bound": "alu", "achieved": ginstr, "peak": ALU_PEAK_GINSTR,
+                                "unit": "Ginstr/s", "frac": ginstr / ALU_PEAK_GINSTR, "traffic": None,
+                                "kernel": "rt_thread_kernel",
+                                "peak_source": "148 SMs x 4 schedulers x 32 lanes x 1.965 GHz (DESIGN.md 7)",
+                                "thread_instructions_per_step": THREAD_INSTR_PER_STEP[args.workload]}
         if not args.no_cpu_baseline and world == 1:
-            sample = max(20, min(firings, int(1e9 // M)))    # ~1e9 reaction-steps: 10-30 s
-            v, dt = oracle_leg(net, x0, seed, traj0, sample)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                    "sample": f"first {sample} firings of {args.workload} "
-                                              f"(M={M}), {dt:.1f} s, single thread"}
+            if n_traj == 1:
+                sample = max(20, min(firings, int(1e9 // M)))    # ~1e9 reaction-steps: 10-30 s
+                v, dt = oracle_leg(net, x0, seed, traj0, sample)
+                line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                        "sample": f"first {sample} firings of {args.workload} "
+                                                  f"(M={M}), {dt:.1f} s, single thread"}
+            else:
+                # ensembles: one independent oracle instance per host core on a subset of the
+                # trajectories, sized for ~1e9 reaction-steps in total
+                import oracle
+                cores = os.cpu_count() or 1
+                per_traj = max(1, fired_per_step // n_traj) * M
+                sub = int(max(cores, min(n_traj, 1e9 // per_traj)))
+                t0 = time.perf_counter()
+                o = oracle.ensemble(net, x0, seed, traj0, sub, firings, t_end, n_threads=cores)
+                dt = time.perf_counter() - t0
+                line["cpu_baseline"] = {"value": float(o["firings"].sum()) / dt, "unit": UNIT,
+                                        "cores": cores, "kind": "oracle",
+                                        "sample": f"trajectories {traj0}..{traj0 + sub - 1} of {args.workload} "
+                                                  f"in full, {dt:.1f} s, one oracle instance per core"}
         print(json.dumps(line))
     model.close()
     if world > 1:
