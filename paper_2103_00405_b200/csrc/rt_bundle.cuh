@@ -915,11 +915,27 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       }
       PT_MARK(2)
       if (SMEM) {
-        if (!is_walker && dirty[tid]) {          // re-scan (read-only) with the new a_k, P_mu
-          dirty[tid] = 0;
-          bool defer = false;
-          best = scan_own<NT, SMEM, false>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, 0.0, false, cnt_pad,
-                                           ctx.any_odd != 0, defer);
+        // re-scan (read-only) with the new a_k, P_mu.  Stale threads are few (usually one, in the
+        // CTA that owns the fired reaction, which is then the last to post), so the thread's warp
+        // shares its reactions: one exact division per lane instead of a serial pass.
+        if (!is_walker) {
+          unsigned stale_mask = __ballot_sync(0xffffffffu, dirty[tid] != 0);
+          if (dirty[tid]) dirty[tid] = 0;
+          if (cnt_pad <= 32 * NT) {
+            while (stale_mask) {
+              const int L = __ffs(stale_mask) - 1;
+              stale_mask &= stale_mask - 1;
+              const int i = (tid - lane + L) + lane * NT;      // lane j: the thread's j-th reaction
+              Cand c = none;
+              if (i < cnt_pad) { c.dt = waiting_time(sP[i], sT[i], sA[i]); c.k = k0 + i; }
+              c = warp_lexmin(c);
+              if (lane == L) best = c;
+            }
+          } else if (stale_mask & (1u << lane)) {
+            bool defer = false;
+            best = scan_own<NT, SMEM, false>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, 0.0, false, cnt_pad,
+                                             ctx.any_odd != 0, defer);
+          }
         }
       } else {
         // State in global memory: one thread re-reading its ~130 strided reactions is a chain of
