@@ -19,6 +19,7 @@ import oracle
 import rt_workloads as W
 from helpers.direct_method import direct_method
 from helpers.exact_kurtz import exact_path
+from helpers.rta_table1 import rta_table1
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 INF = math.inf
@@ -314,3 +315,20 @@ def test_agrees_in_distribution_with_direct_method(case):
     xd, _ = direct_method(net, x0, n_traj, t_end, seed=1234)
     for j in range(net["n_species"]):
         _two_sample(out["x"][:, j].astype(float), xd[:, j].astype(float))
+
+
+@pytest.mark.parametrize("case", ["birth_death", "dimer", "lv"])
+def test_agrees_in_distribution_with_table1_random_time_algorithm(case):
+    """Pin P10: the next-reaction form (one new random per firing, Eq.26) and the paper's Table 1
+    (M fresh randoms every step) are the same process: marginals at t_end agree."""
+    if case == "birth_death":
+        (net, x0), t_end, n_traj = W.birth_death(), 30.0, 2000
+    elif case == "dimer":
+        net = W.from_reactions(2, [({0: 2}, {1: 1}, 0.01), ({1: 1}, {0: 2}, 1.0)])
+        x0, t_end, n_traj = [100, 0], 2.0, 2000
+    else:
+        (net, x0), t_end, n_traj = W.lotka_volterra(), 0.3, 1500
+    out = oracle.ensemble(net, x0, seed=91, traj_first=0, n_traj=n_traj, t_end=t_end, n_threads=4)
+    xt = rta_table1(net, x0, n_traj, t_end, seed=4321)
+    for j in range(net["n_species"]):
+        _two_sample(out["x"][:, j].astype(float), xt[:, j].astype(float))
