@@ -103,6 +103,33 @@ def test_hub_species_general_rows_and_staging_overflow(rt, ctas, state_mode):
                             ("refresh_mode", refresh_mode)])
 
 
+@pytest.mark.parametrize("ctas", [1, 0])
+def test_extreme_rates_and_cubic_reactions(rt, ctas):
+    """Rates from 1e-300 to 1e300 (outside the range where the approximate-quotient filter of the
+    scan is proven, so the exact path must take over), zero and negative-zero rates, and
+    trimolecular 3A -> B reactions (sigma = 3, count bound 2^21 - 1)."""
+    rng = np.random.default_rng(11)
+    n_species, reactions = 30, []
+    for k in range(1500):
+        j = [int(v) for v in rng.choice(n_species, size=3, replace=False)]
+        kind = k % 6
+        if kind == 0:
+            reactions.append(({j[0]: 3}, {j[1]: 1}, float(10.0 ** rng.uniform(-6, -3))))
+        elif kind == 1:
+            reactions.append(({j[0]: 1, j[1]: 2}, {j[2]: 1}, float(10.0 ** rng.uniform(-300, -250))))
+        elif kind == 2:
+            reactions.append(({j[0]: 1}, {j[1]: 1}, float(10.0 ** rng.uniform(250, 300))))
+        elif kind == 3:
+            reactions.append(({j[0]: 1}, {j[1]: 2}, 0.0 if k % 12 == 3 else -0.0))
+        else:
+            reactions.append(({j[0]: 1, j[1]: 1}, {j[2]: 1, j[0]: 1}, float(10.0 ** rng.uniform(-2, 1))))
+    net = W.from_reactions(n_species, reactions)
+    x0 = rng.integers(5, 40, size=n_species).astype(np.int64)
+    for state_mode in (0, 1):
+        _check_run(rt, net, x0, 31, 2, 800, math.inf, 800,
+                   options=[("bundle_ctas", ctas), ("state_mode", state_mode)])
+
+
 def test_count_overflow_is_reported(rt):
     """0 -> X from the count bound: after the three deaths of the other species the first birth
     leaves [0, 2^31-1] -> RT_ERR_OVERFLOW at firing 4."""
