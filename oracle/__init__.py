@@ -27,6 +27,7 @@ def lib():
         _lib.oracle_binom.restype = C.c_int64
         _lib.oracle_binom.argtypes = [C.c_int64, C.c_int32]
         _lib.oracle_run.restype = C.c_int
+        _lib.oracle_run_residual.restype = C.c_int
         _lib.oracle_ensemble.restype = C.c_int
     return _lib
 
@@ -104,6 +105,33 @@ def run(net, x0, seed, trajectory=0, max_firings=0, t_end=math.inf, trace_cap=0,
     nrec = min(int(firings.value), trace_cap)
     return dict(x=x, t=t.value, firings=int(firings.value), stop=int(stop.value), code=rc,
                 fire_count=fc, T=T, P=P,
+                trace_mu=None if tmu is None else tmu[:nrec],
+                trace_t=None if tt is None else tt[:nrec])
+
+
+def run_residual(net, x0, seed, trajectory=0, max_firings=0, t_end=math.inf, trace_cap=0):
+    """One trajectory of the residual (Table 3) form.  Returns x, t, firings, stop, fire_count, R,
+    trace_mu, trace_t."""
+    args, keep = _net_args(net)
+    N, M = int(net["n_species"]), int(net["n_reactions"])
+    x0 = np.ascontiguousarray(x0, dtype=np.int64)
+    x = np.zeros(N, dtype=np.int64)
+    t = C.c_double(0.0)
+    firings = C.c_uint64(0)
+    stop = C.c_int32(0)
+    fc = np.zeros(M, dtype=np.uint64)
+    R = np.zeros(M, dtype=np.float64)
+    tmu = np.zeros(trace_cap, dtype=np.int32) if trace_cap else None
+    tt = np.zeros(trace_cap, dtype=np.float64) if trace_cap else None
+    rc = lib().oracle_run_residual(*args, _p(x0, C.c_int64), C.c_uint64(seed), C.c_uint64(trajectory),
+                                   C.c_uint64(max_firings), C.c_double(t_end), _p(x, C.c_int64),
+                                   C.byref(t), C.byref(firings), C.byref(stop), _p(fc, C.c_uint64),
+                                   _p(R, C.c_double), _p(tmu, C.c_int32), _p(tt, C.c_double),
+                                   C.c_uint64(trace_cap))
+    if rc != 0:
+        raise RuntimeError(f"oracle_run_residual failed with code {rc}")
+    nrec = min(int(firings.value), trace_cap)
+    return dict(x=x, t=t.value, firings=int(firings.value), stop=int(stop.value), fire_count=fc, R=R,
                 trace_mu=None if tmu is None else tmu[:nrec],
                 trace_t=None if tt is None else tt[:nrec])
 

@@ -25,6 +25,7 @@
 //                    Eq.5 X += v_mu.
 //                    Table 2 (the NRRTA listing) lost its body in PAPER.md:258-260; the
 //                    (T_k, P_k) bookkeeping is reading G3 of DESIGN.md.
+//   nrrta_run_residual()  Table 3 in residual-internal-time form (reading G4)
 //   direct-method cross-check lives in tests/ (it must not share code with this file).
 //
 // Parity pins (tests/test_oracle_*.py): Philox known-answer vectors and the CUDA toolkit's
@@ -198,6 +199,85 @@ int nrrta_run(const Net &net, const int64_t *x0, uint64_t seed, uint64_t traj,
   return rc;
 }
 
+
+// ---------------------------------------------------------------- residual ("Table 3") form
+// PAPER.md Table 3 (:262-272), the memory-lean parallel listing: per channel only the remaining
+// real waiting time is kept and rescaled, Delta t_k <- (p_k / a_k)(Delta t_k - Delta t_mu) with
+// p_k the previous propensity, and the fired channel draws Delta t_mu = ln(1/r) / a_mu.
+// Reading G4: written with the residual INTERNAL time R_k = a_k^old (Delta t_k - Delta t_mu)
+// = P_k - T_k it is the same process without the division by a_k = 0:
+//     Delta t_k = R_k / a_k,   R_k <- R_k - a_k * Delta t_mu for every k,   R_mu <- ln(1/r).
+// Same law as nrrta_run, different rounding (one array instead of two), so sample paths differ
+// in the last bits and eventually in the fired sequence: its own parity target.
+int nrrta_run_residual(const Net &net, const int64_t *x0, uint64_t seed, uint64_t traj,
+                       uint64_t max_firings, double t_end,
+                       int64_t *x_out, double *t_out, uint64_t *firings_out, int32_t *stop_out,
+                       uint64_t *fire_count_out, double *R_out,
+                       int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
+  const int32_t M = net.M, N = net.N;
+  const double INF = std::numeric_limits<double>::infinity();
+  const int64_t xmax = count_bound(net);
+  for (int64_t e = 0; e < net.react_ptr[M]; ++e)
+    if (net.react_sigma[e] < 1 || net.react_sigma[e] > 3) return ERR_BAD;
+  std::vector<int64_t> X(x0, x0 + N);
+  for (int32_t j = 0; j < N; ++j) if (X[j] < 0 || X[j] > xmax) return ERR_BAD;
+  std::vector<double> R(M), a(M), dt(M);
+  std::vector<uint32_t> n(M, 0u);
+  for (int32_t k = 0; k < M; ++k) R[k] = exp_draw(seed, traj, (uint32_t)k, 0u);
+  double t = 0.0;
+  uint64_t fired = 0;
+  int32_t stop = 0;
+  int rc = OK;
+  for (;;) {
+    for (int32_t k = 0; k < M; ++k) a[k] = propensity(net, X.data(), k);
+    for (int32_t k = 0; k < M; ++k) {
+      if (a[k] > 0.0) {
+        double r = R[k];
+        if (r < 0.0) r = 0.0;          // reading G7
+        dt[k] = r / a[k];
+      } else {
+        dt[k] = INF;
+      }
+    }
+    int32_t mu = 0;
+    double delta = dt[0];
+    for (int32_t k = 1; k < M; ++k)
+      if (dt[k] < delta) { delta = dt[k]; mu = k; }
+    if (delta == INF) { stop = STOP_ABSORBED; break; }
+    if (t_end < INF && t + delta > t_end) {
+      const double rest = t_end - t;
+      for (int32_t k = 0; k < M; ++k) { const double dec = a[k] * rest; R[k] = R[k] - dec; }
+      t = t_end;
+      stop = STOP_T_END;
+      break;
+    }
+    t = t + delta;
+    for (int32_t k = 0; k < M; ++k) { const double dec = a[k] * delta; R[k] = R[k] - dec; }
+    for (int64_t e = net.stoich_ptr[mu]; e < net.stoich_ptr[mu + 1]; ++e) {
+      int64_t &xj = X[net.stoich_species[e]];
+      xj += net.stoich_v[e];
+      if (xj < 0) rc = ERR_BAD;
+      if (xj > xmax) rc = ERR_OVERFLOW;
+    }
+    n[mu] += 1u;
+    R[mu] = exp_draw(seed, traj, (uint32_t)mu, n[mu]);     // Table 3: a fresh ln(1/r) for mu only
+    if (fired < trace_cap) {
+      if (trace_mu) trace_mu[fired] = mu;
+      if (trace_t) trace_t[fired] = t;
+    }
+    fired += 1;
+    if (rc != OK) break;
+    if (max_firings != 0 && fired == max_firings) { stop = STOP_MAX_FIRINGS; break; }
+  }
+  if (x_out) for (int32_t j = 0; j < N; ++j) x_out[j] = X[j];
+  if (t_out) *t_out = t;
+  if (firings_out) *firings_out = fired;
+  if (stop_out) *stop_out = stop;
+  if (fire_count_out) for (int32_t k = 0; k < M; ++k) fire_count_out[k] = n[k];
+  if (R_out) for (int32_t k = 0; k < M; ++k) R_out[k] = R[k];
+  return rc;
+}
+
 }  // namespace
 
 extern "C" {
@@ -229,6 +309,18 @@ int oracle_run(int32_t N, int32_t M, const int64_t *react_ptr, const int32_t *re
   Net net{N, M, react_ptr, react_species, react_sigma, stoich_ptr, stoich_species, stoich_v, rate};
   return nrrta_run(net, x0, seed, traj, max_firings, t_end, x_out, t_out, firings_out,
                    stop_out, fire_count_out, T_out, P_out, trace_mu, trace_t, trace_cap);
+}
+
+int oracle_run_residual(int32_t N, int32_t M, const int64_t *react_ptr, const int32_t *react_species,
+                        const int32_t *react_sigma, const int64_t *stoich_ptr,
+                        const int32_t *stoich_species, const int32_t *stoich_v, const double *rate,
+                        const int64_t *x0, uint64_t seed, uint64_t traj, uint64_t max_firings,
+                        double t_end, int64_t *x_out, double *t_out, uint64_t *firings_out,
+                        int32_t *stop_out, uint64_t *fire_count_out, double *R_out,
+                        int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
+  Net net{N, M, react_ptr, react_species, react_sigma, stoich_ptr, stoich_species, stoich_v, rate};
+  return nrrta_run_residual(net, x0, seed, traj, max_firings, t_end, x_out, t_out, firings_out,
+                            stop_out, fire_count_out, R_out, trace_mu, trace_t, trace_cap);
 }
 
 // Independent trajectories traj_first .. traj_first+n_traj-1, each by the single-threaded

@@ -332,3 +332,45 @@ def test_agrees_in_distribution_with_table1_random_time_algorithm(case):
     xt = rta_table1(net, x0, n_traj, t_end, seed=4321)
     for j in range(net["n_species"]):
         _two_sample(out["x"][:, j].astype(float), xt[:, j].astype(float))
+
+
+# ------------------------------------------------------------------ residual (Table 3) form
+def test_residual_form_single_source_closed_form():
+    """Table 3: one source channel, a = c constant, so Delta t_i = E_i / c and
+    t_n = sum_i fl(E_i / c) with the same draws E(seed, traj, 0, i) as the (T, P) form."""
+    c = 2.5
+    net = W.from_reactions(1, [({}, {0: 1}, c)])
+    o = oracle.run_residual(net, [0], seed=9, trajectory=4, max_firings=200, trace_cap=200)
+    t = 0.0
+    for i in range(200):
+        t = t + oracle.exp_draw(9, 4, 0, i) / c
+        assert o["trace_t"][i] == t
+    assert o["x"][0] == 200 and o["firings"] == 200
+
+
+def test_residual_form_tie_rule_kurtz_and_t_end():
+    net, x0, par = W.make_config("cfg3", scale=0.01)
+    o = oracle.run_residual(net, x0, par["seed"], 0, 0, 0.002, 4096)
+    assert o["stop"] == oracle.STOP_T_END and o["t"] == 0.002
+    V = np.zeros((net["n_reactions"], net["n_species"]), dtype=np.int64)
+    for k in range(net["n_reactions"]):
+        for e in range(net["stoich_ptr"][k], net["stoich_ptr"][k + 1]):
+            V[k, net["stoich_species"][e]] = net["stoich_v"][e]
+    np.testing.assert_array_equal(o["x"], np.asarray(x0) + o["fire_count"].astype(np.int64) @ V)   # Eq.5
+    assert o["fire_count"].sum() == o["firings"] and (np.diff(o["trace_t"]) >= 0).all() and (o["x"] >= 0).all()
+    # two identical channels, identical first draws impossible -> but a = 0 everywhere is a tie at +inf
+    dead = W.from_reactions(1, [({0: 1}, {}, 1.0), ({0: 2}, {}, 1.0)])
+    assert oracle.run_residual(dead, [0], 1, 0, 10)["stop"] == oracle.STOP_ABSORBED
+
+
+@pytest.mark.parametrize("case", ["birth_death", "lv"])
+def test_residual_form_agrees_in_distribution_with_direct_method(case):
+    """Same process as the (T, P) form and as Gillespie's direct method."""
+    if case == "birth_death":
+        (net, x0), t_end, n_traj = W.birth_death(), 30.0, 1500
+    else:
+        (net, x0), t_end, n_traj = W.lotka_volterra(), 0.3, 1200
+    xs = np.array([oracle.run_residual(net, x0, 55, i, 0, t_end)["x"] for i in range(n_traj)])
+    xd, _ = direct_method(net, x0, n_traj, t_end, seed=999)
+    for j in range(net["n_species"]):
+        _two_sample(xs[:, j].astype(float), xd[:, j].astype(float))
