@@ -132,7 +132,7 @@ int rt_ensemble_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t 
  * reported a barrier timeout or the runtime reported an error. */
 int rt_sync(rt_model *m, void *stream);
 
-/* Tuning / debug knobs (all optional; results never depend on them).
+/* Tuning / debug knobs (all optional; results never depend on them, except "formulation").
  *   "refresh_mode"   0 = dependency-graph refresh of a_k (default), 1 = recompute every a_k
  *                    each firing (the paper's own GPU scheme)
  *   "bundle_ctas"    CTAs cooperating on one trajectory; 0 = choose automatically
@@ -142,6 +142,10 @@ int rt_sync(rt_model *m, void *stream);
  *                    1 = always stream it from global memory (the regime of M > ~1.1e6)
  *   "prefetch"       bit 0: L2 prefetch of the candidate's walk data, bit 1: speculative redraw,
  *                    bit 2: pre-walk of the exchange's runner-up (default 7 = all)
+ *   "formulation"    0 = (T_k, P_k) internal-time form (default; the form every parity claim is
+ *                    made for), 1 = residual form of PAPER.md Table 3 (R_k = P_k - T_k kept in one
+ *                    array: T_out then holds -R_k and P_out zeros).  Same process, different
+ *                    rounding: its sample paths match oracle_run_residual, not oracle_run.
  *   "x_replicas"     copies of X per trajectory the CTAs spread their updates over (default 1)
  * Returns RT_ERR_BAD_ARG for an unknown name or value. */
 int rt_set_option(rt_model *m, const char *name, int64_t value);

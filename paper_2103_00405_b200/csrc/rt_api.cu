@@ -72,7 +72,7 @@ struct rt_model {
   // staging for the host-pointer API
   DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t;
   // options
-  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0, opt_prefetch = 7;
+  int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0, opt_prefetch = 7, opt_formulation = 0;
   // info
   int64_t kernel_launches = 0;
   int last_S = 0, last_B = 0, last_path = 0, last_state_smem = 0;
@@ -210,6 +210,7 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.trace_cap = (trace_mu_dev || trace_t_dev) ? trace_cap : 0;
   p.refresh_mode = m->refresh_mode;
   p.prefetch = m->opt_prefetch;
+  p.formulation = m->opt_formulation;
   p.err = (int *)m->d_err.p;
   void *args[] = {&p};
   // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
@@ -475,7 +476,7 @@ int rt_ensemble_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t 
   if (rc != RT_OK) return rc;
   if (n_traj == 0) return RT_OK;
   CU_TRY(cudaSetDevice(m->device));
-  bool use_threads = thread_path_fits(m);
+  bool use_threads = thread_path_fits(m) && m->opt_formulation == 0;   // (the thread kernel is (T,P) only)
   if (m->opt_ensemble_path == 1) {
     if (!thread_path_fits(m)) return RT_ERR_BAD_ARG;
     use_threads = true;
@@ -533,6 +534,9 @@ int rt_set_option(rt_model *m, const char *name, int64_t value) {
   } else if (!strcmp(name, "ensemble_path")) {
     if (value < 0 || value > 2) return RT_ERR_BAD_ARG;
     m->opt_ensemble_path = (int)value;
+  } else if (!strcmp(name, "formulation")) {
+    if (value < 0 || value > 1) return RT_ERR_BAD_ARG;
+    m->opt_formulation = (int)value;
   } else if (!strcmp(name, "prefetch")) {
     if (value < 0 || value > 7) return RT_ERR_BAD_ARG;
     m->opt_prefetch = (int)value;

@@ -59,6 +59,8 @@ struct BundleParams {
   double *trace_t;
   u64 trace_cap;
   int prefetch;           // walker prefetches its candidate's walk data during the exchange
+  int formulation;        // 0: (T, P) internal-time form; 1: residual (Table 3) form, kept as
+                          //    T_k = -R_k with P_k = 0 (same operations, one array less to read)
   int refresh_mode;       // 0 dependency walk, 1 recompute every a_k (the paper's GPU scheme)
   int *err;               // set to 1 on a barrier timeout
 };
@@ -184,7 +186,8 @@ __device__ __forceinline__ Cand scan_filtered(int tid, int k0, int cnt_pad, doub
 // reactions per thread and iteration, i.e. twelve 16-byte loads (192 B) in flight per thread
 // before any is used, and ~1/3 of the instructions of dividing everything, so that the pass is
 // bound by the memory system and not by issue slots.  Padding reactions (k >= M) hold a = 0.
-template <int NT, bool UPDATE>
+// RESID: residual form -- P is identically 0 and is not read (24 instead of 32 bytes per reaction).
+template <int NT, bool UPDATE, bool RESID>
 __device__ __forceinline__ Cand scan_filtered_global(int tid, int k0, int k1, double *T, double *P,
                                                      double *A, double dprev, bool any_odd, bool &defer) {
   constexpr int U = 4;
@@ -200,8 +203,14 @@ __device__ __forceinline__ Cand scan_filtered_global(int tid, int k0, int k1, do
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int qu = q + u * NT;
-      if (qu < q1) { tt[u] = __ldcg(T2 + qu); pp[u] = __ldcg(P2 + qu); aa[u] = __ldcg(A2 + qu); }
-      else { tt[u] = make_double2(0.0, 0.0); pp[u] = make_double2(1.0, 1.0); aa[u] = tt[u]; }  // q~ = +inf
+      if (qu < q1) {
+        tt[u] = __ldcg(T2 + qu); aa[u] = __ldcg(A2 + qu);
+        pp[u] = RESID ? make_double2(0.0, 0.0) : __ldcg(P2 + qu);
+      } else {                                   // P - T = 1, a = 0: q~ = +inf
+        tt[u] = make_double2(RESID ? -1.0 : 0.0, RESID ? -1.0 : 0.0);
+        pp[u] = make_double2(RESID ? 0.0 : 1.0, RESID ? 0.0 : 1.0);
+        aa[u] = make_double2(0.0, 0.0);
+      }
     }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
@@ -225,7 +234,7 @@ __device__ __forceinline__ Cand scan_filtered_global(int tid, int k0, int k1, do
   const float thr = m1 * (1.0f + kFilterTol);
   const bool decided = !any_odd && m1 >= 0x1.0p-100f && m1 <= 0x1.0p100f && m2 > thr;
   if (decided) {
-    best.dt = waiting_time(__ldcg(P + i1), __ldcg(T + i1), __ldcg(A + i1));
+    best.dt = waiting_time(RESID ? 0.0 : __ldcg(P + i1), __ldcg(T + i1), __ldcg(A + i1));
     best.k = i1;
   } else if (UPDATE) {
     defer = true;                               // left to the re-scan (see scan_filtered)
@@ -256,12 +265,14 @@ template <int NT, bool SMEM, bool UPDATE>
 __device__ __forceinline__ Cand scan_own(const NetDev &net, const u64 *X, int tid, int k0, int k1,
                                          double *sT, const double *sP, double *sA,
                                          double *T, double *P, double *A, double dprev, bool full,
-                                         int cnt_pad, bool any_odd, bool &defer) {
+                                         int cnt_pad, bool any_odd, bool &defer, bool resid = false) {
   Cand best;
   best.dt = __longlong_as_double(0x7ff0000000000000ll);
   best.k = 0x7fffffff;
   if (SMEM && !full) return scan_filtered<NT, UPDATE>(tid, k0, cnt_pad, sT, sP, sA, dprev, any_odd, defer);
-  if (!SMEM && !full) return scan_filtered_global<NT, UPDATE>(tid, k0, k1, T, P, A, dprev, any_odd, defer);
+  if (!SMEM && !full)
+    return resid ? scan_filtered_global<NT, UPDATE, true>(tid, k0, k1, T, P, A, dprev, any_odd, defer)
+                 : scan_filtered_global<NT, UPDATE, false>(tid, k0, k1, T, P, A, dprev, any_odd, defer);
   if (SMEM) {
     const int cnt = k1 - k0;
 #pragma unroll 4
@@ -541,8 +552,12 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
     }
     if (c.k < p.net.M && c.k != spec.k && lane == 0 && (p.prefetch & 2)) {
       const uint32_t n1 = nfire[c.k] + 1u;
-      const double pold = spec.sP ? spec.sP[c.k - spec.k0] : __ldcg(spec.P_glob + c.k);
-      spec.P = __dadd_rn(pold, exp_draw(spec.seed, spec.traj, (uint32_t)c.k, n1));
+      if (p.formulation) {
+        spec.P = -exp_draw(spec.seed, spec.traj, (uint32_t)c.k, n1);       // residual form: T_k = -E
+      } else {
+        const double pold = spec.sP ? spec.sP[c.k - spec.k0] : __ldcg(spec.P_glob + c.k);
+        spec.P = __dadd_rn(pold, exp_draw(spec.seed, spec.traj, (uint32_t)c.k, n1));
+      }
       spec.n = n1;
       spec.k = c.k;
     }
@@ -629,6 +644,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   const int b = blockIdx.x / p.S, r = blockIdx.x % p.S;
   const int M = net.M, N = net.N;
   const double INF = __longlong_as_double(0x7ff0000000000000ll);
+  const bool resid = p.formulation != 0;
 
   double *T = p.T + (size_t)b * net.M_pad;
   double *P = p.P + (size_t)b * net.M_pad;
@@ -676,8 +692,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         p0 = exp_draw(p.seed, traj, (uint32_t)k, 0u);
         if (filter_unsafe(a0)) ctx.any_odd = 1;
       }
-      if (SMEM) { sT[k - k0] = 0.0; sP[k - k0] = p0; sA[k - k0] = a0; }
-      else { __stcg(T + k, 0.0); __stcg(P + k, p0); __stcg(A + k, a0); }
+      const double t_init = resid ? -p0 : 0.0, p_init = resid ? 0.0 : p0;   // residual form: T = -R
+      if (SMEM) { sT[k - k0] = t_init; sP[k - k0] = p_init; sA[k - k0] = a0; }
+      else { __stcg(T + k, t_init); __stcg(P + k, p_init); __stcg(A + k, a0); }
       if (k < k1) nfire[k] = 0u;
     }
     __syncthreads();
@@ -819,7 +836,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
               ctx.p_val = spec.P;
             } else {
               nfire[mu_prev] = c_old + 1u;
-              ctx.p_val = __dadd_rn(p_old, exp_draw(p.seed, traj, (uint32_t)mu_prev, c_old + 1u));
+              const double e_new = exp_draw(p.seed, traj, (uint32_t)mu_prev, c_old + 1u);
+              ctx.p_val = resid ? -e_new : __dadd_rn(p_old, e_new);
             }
             ctx.p_k = mu_prev;
             spec.k = -1;
@@ -868,7 +886,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           // ===== stream warps: a-5 of the previous firing fused with a-2/a-3 of this one =====
           bool defer = false;
           best = scan_own<NT, SMEM, true>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, dprev, full, cnt_pad,
-                                          ctx.any_odd != 0, defer);
+                                          ctx.any_odd != 0, defer, resid);
           mybest_k[tid] = defer ? -3 : best.k;
           if (defer) dirty[tid] = 1;
         }
@@ -904,7 +922,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         }
         if (tid == 0) {
           if (first_round && pk_now >= 0) {
-            if (SMEM) sP[pk_now - k0] = ctx.p_val; else __stcg(P + pk_now, ctx.p_val);
+            if (resid) { if (SMEM) sT[pk_now - k0] = ctx.p_val; else __stcg(T + pk_now, ctx.p_val); }
+            else { if (SMEM) sP[pk_now - k0] = ctx.p_val; else __stcg(P + pk_now, ctx.p_val); }
             dirty[owner_thread<NT, SMEM>(pk_now, k0)] = 1;
           }
           ctx.n_stale = 0;

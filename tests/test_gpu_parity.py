@@ -315,3 +315,54 @@ def test_cfg2_ensemble_statistics(rt):
     assert ps[0] > 0.01 / 2 and ps[1] > 0.01      # Holm-corrected
     fz = _ks_and_moments(other["firings"].astype(float), o["firings"].astype(float))[1]
     assert fz < 3.0
+
+
+# ------------------------------------------------------------------ residual (Table 3) formulation
+def _check_residual(rt, net, x0, seed, traj, max_firings, t_end, trace_cap, options=()):
+    o = _oracle().run_residual(net, x0, seed, traj, max_firings, t_end, trace_cap)
+    with rt.Model(net) as m:
+        m.set_option("formulation", 1)
+        for name, val in options:
+            m.set_option(name, val)
+        g = m.run(x0, seed, traj, max_firings, t_end, trace_cap, want_state=True)
+    assert g["firings"] == o["firings"] and g["stop"] == o["stop"]
+    np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["fire_count"], o["fire_count"])
+    np.testing.assert_allclose(g["trace_t"], o["trace_t"], rtol=RTOL_T, atol=0)
+    # T_out holds -R_k, P_out zeros
+    np.testing.assert_allclose(-g["T"], o["R"], rtol=1e-10, atol=1e-12)
+    assert not g["P"].any()
+    return g, o
+
+
+@pytest.mark.parametrize("ctas,state_mode", [(0, 0), (3, 0), (0, 1), (1, 1)])
+def test_residual_form_matches_its_oracle(rt, ctas, state_mode):
+    """PAPER.md Table 3 in residual form (formulation = 1) against oracle_run_residual: fired
+    sequence and counts bit-exact, times to 1e-12 -- with the state in shared memory and streamed
+    from global memory (where P is not read at all: 24 instead of 32 bytes per reaction)."""
+    net, x0, par = W.make_config("cfg3", scale=0.03)
+    _check_residual(rt, net, x0, par["seed"], 1, 1500, math.inf, 1500,
+                    options=[("bundle_ctas", ctas), ("state_mode", state_mode)])
+    net, x0 = _hub_network()
+    _check_residual(rt, net, x0, 21, 0, 400, math.inf, 400,
+                    options=[("bundle_ctas", ctas), ("state_mode", state_mode)])
+
+
+def test_residual_form_stops_and_full_recompute(rt):
+    net, x0, par = W.make_config("cfg3", scale=0.01)
+    g, o = _check_residual(rt, net, x0, 11, 0, 0, 0.002, 4096)
+    assert g["stop"] == rt.RT_STOP_T_END and g["t"] == 0.002
+    _check_residual(rt, net, x0, 11, 0, 700, math.inf, 700, options=[("refresh_mode", 1)])
+    net, x0 = W.lotka_volterra()
+    _check_residual(rt, net, x0, 5, 9, 2000, math.inf, 2000)
+
+
+def test_residual_form_cfg4_prefix_and_differs_from_default(rt):
+    """Bench shape (M = 1e6): 1500 firings against the residual oracle.  The two formulations
+    are the same process but round differently, so their paths eventually part."""
+    net, x0, par = W.make_config("cfg4")
+    g, o = _check_residual(rt, net, x0, par["seed"], 0, 1500, math.inf, 1500)
+    with rt.Model(net) as m:
+        d = m.run(x0, par["seed"], 0, 1500, trace_cap=1500)
+    assert d["trace_mu"][0] == g["trace_mu"][0]          # same first draws -> same first firing
