@@ -28,6 +28,7 @@ def lib():
         _lib.oracle_binom.argtypes = [C.c_int64, C.c_int32]
         _lib.oracle_run.restype = C.c_int
         _lib.oracle_run_residual.restype = C.c_int
+        _lib.oracle_run_sched.restype = C.c_int
         _lib.oracle_ensemble.restype = C.c_int
     return _lib
 
@@ -105,6 +106,40 @@ def run(net, x0, seed, trajectory=0, max_firings=0, t_end=math.inf, trace_cap=0,
     nrec = min(int(firings.value), trace_cap)
     return dict(x=x, t=t.value, firings=int(firings.value), stop=int(stop.value), code=rc,
                 fire_count=fc, T=T, P=P,
+                trace_mu=None if tmu is None else tmu[:nrec],
+                trace_t=None if tt is None else tt[:nrec])
+
+
+def run_sched(net, x0, seed, trajectory=0, max_firings=0, t_end=math.inf, trace_cap=0,
+              t_break=(), factor=(), mask=None):
+    """One trajectory with piecewise-constant rate modulation (Eq.28): c_k(t) = c_k *
+    factor[i] for t in [t_break[i], t_break[i+1]) for the channels with mask[k] != 0 (all if None)."""
+    args, keep = _net_args(net)
+    N, M = int(net["n_species"]), int(net["n_reactions"])
+    x0 = np.ascontiguousarray(x0, dtype=np.int64)
+    tb = np.ascontiguousarray(t_break, dtype=np.float64)
+    fa = np.ascontiguousarray(factor, dtype=np.float64)
+    assert tb.shape == fa.shape
+    mk = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    x = np.zeros(N, dtype=np.int64)
+    t = C.c_double(0.0)
+    firings = C.c_uint64(0)
+    stop = C.c_int32(0)
+    fc = np.zeros(M, dtype=np.uint64)
+    T = np.zeros(M, dtype=np.float64)
+    P = np.zeros(M, dtype=np.float64)
+    tmu = np.zeros(trace_cap, dtype=np.int32) if trace_cap else None
+    tt = np.zeros(trace_cap, dtype=np.float64) if trace_cap else None
+    rc = lib().oracle_run_sched(*args, _p(x0, C.c_int64), C.c_uint64(seed), C.c_uint64(trajectory),
+                                C.c_uint64(max_firings), C.c_double(t_end), C.c_int32(len(tb)),
+                                _p(tb, C.c_double), _p(fa, C.c_double), _p(mk, C.c_uint8),
+                                _p(x, C.c_int64), C.byref(t), C.byref(firings), C.byref(stop),
+                                _p(fc, C.c_uint64), _p(T, C.c_double), _p(P, C.c_double),
+                                _p(tmu, C.c_int32), _p(tt, C.c_double), C.c_uint64(trace_cap))
+    if rc != 0:
+        raise RuntimeError(f"oracle_run_sched failed with code {rc}")
+    nrec = min(int(firings.value), trace_cap)
+    return dict(x=x, t=t.value, firings=int(firings.value), stop=int(stop.value), fire_count=fc, T=T, P=P,
                 trace_mu=None if tmu is None else tmu[:nrec],
                 trace_t=None if tt is None else tt[:nrec])
 

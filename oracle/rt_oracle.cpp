@@ -25,6 +25,7 @@
 //                    Eq.5 X += v_mu.
 //                    Table 2 (the NRRTA listing) lost its body in PAPER.md:258-260; the
 //                    (T_k, P_k) bookkeeping is reading G3 of DESIGN.md.
+//   nrrta_run_sched()     Eq.28 with piecewise-constant c_k(t)
 //   nrrta_run_residual()  Table 3 in residual-internal-time form (reading G4)
 //   direct-method cross-check lives in tests/ (it must not share code with this file).
 //
@@ -278,6 +279,113 @@ int nrrta_run_residual(const Net &net, const int64_t *x0, uint64_t seed, uint64_
   return rc;
 }
 
+
+// ---------------------------------------------------------------- time-dependent rates
+// PAPER.md section 6, Eq.28 (:224-231): with rates c_k(s) that depend on time, channel k fires when
+//     h_k * int_t^{t+dt_k} c_k(s) ds = P_k - T_k,        h_k = prod_j C(X_j, sigma_jk),
+// and "the integral can be calculated analytically for well behaved time-dependent reaction
+// rates" (:229).  The family built here is piecewise-constant modulation: c_k(s) = c_k * f_i for
+// s in [b_i, b_{i+1}) (f = 1 before b_0) for the channels selected by `mask` (all if NULL), the
+// others keep c_k.  The integral is then piecewise linear, so between two breakpoints the step
+// is Eq.24 unchanged, and a step that would cross the next breakpoint b is cut there:
+// T_k += a_k (b - t) for every k, t = b, no firing, rates switch to the next factor.
+// The effective rate is one rounded product RN(c_k * f_i), then Eq.1-2 as before.
+double propensity_eff(const Net &net, const int64_t *X, int32_t k, double f, const uint8_t *mask) {
+  double a = net.rate[k];
+  if (mask == nullptr || mask[k]) a = a * f;
+  for (int64_t e = net.react_ptr[k]; e < net.react_ptr[k + 1]; ++e) {
+    const int64_t b = binom(X[net.react_species[e]], net.react_sigma[e]);
+    a = a * (double)b;
+  }
+  return a;
+}
+
+int nrrta_run_sched(const Net &net, const int64_t *x0, uint64_t seed, uint64_t traj,
+                    uint64_t max_firings, double t_end,
+                    int32_t n_break, const double *t_break, const double *factor, const uint8_t *mask,
+                    int64_t *x_out, double *t_out, uint64_t *firings_out, int32_t *stop_out,
+                    uint64_t *fire_count_out, double *T_out, double *P_out,
+                    int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
+  const int32_t M = net.M, N = net.N;
+  const double INF = std::numeric_limits<double>::infinity();
+  const int64_t xmax = count_bound(net);
+  for (int64_t e = 0; e < net.react_ptr[M]; ++e)
+    if (net.react_sigma[e] < 1 || net.react_sigma[e] > 3) return ERR_BAD;
+  for (int32_t i = 0; i < n_break; ++i) {
+    if (!(t_break[i] >= 0.0) || !(factor[i] >= 0.0) || factor[i] == INF || t_break[i] == INF) return ERR_BAD;
+    if (i > 0 && !(t_break[i] > t_break[i - 1])) return ERR_BAD;
+  }
+  std::vector<int64_t> X(x0, x0 + N);
+  for (int32_t j = 0; j < N; ++j) if (X[j] < 0 || X[j] > xmax) return ERR_BAD;
+  std::vector<double> T(M, 0.0), P(M), a(M), dt(M);
+  std::vector<uint32_t> n(M, 0u);
+  for (int32_t k = 0; k < M; ++k) P[k] = exp_draw(seed, traj, (uint32_t)k, 0u);
+  double t = 0.0, f = 1.0;
+  int32_t seg = 0;                      // breakpoints already passed
+  uint64_t fired = 0;
+  int32_t stop = 0;
+  int rc = OK;
+  for (;;) {
+    for (int32_t k = 0; k < M; ++k) a[k] = propensity_eff(net, X.data(), k, f, mask);
+    for (int32_t k = 0; k < M; ++k) {
+      if (a[k] > 0.0) {
+        double r = P[k] - T[k];
+        if (r < 0.0) r = 0.0;
+        dt[k] = r / a[k];
+      } else {
+        dt[k] = INF;
+      }
+    }
+    int32_t mu = 0;
+    double delta = dt[0];
+    for (int32_t k = 1; k < M; ++k)
+      if (dt[k] < delta) { delta = dt[k]; mu = k; }
+    // the next breakpoint (if it lies within the run) cuts the step
+    const double tb = (seg < n_break && t_break[seg] <= t_end) ? t_break[seg] : INF;
+    if (tb < INF && (delta == INF || t + delta > tb)) {
+      const double rest = tb - t;
+      for (int32_t k = 0; k < M; ++k) { const double inc = a[k] * rest; T[k] = T[k] + inc; }
+      t = tb;
+      f = factor[seg];
+      seg += 1;
+      continue;
+    }
+    if (delta == INF) { stop = STOP_ABSORBED; break; }
+    if (t_end < INF && t + delta > t_end) {
+      const double rest = t_end - t;
+      for (int32_t k = 0; k < M; ++k) { const double inc = a[k] * rest; T[k] = T[k] + inc; }
+      t = t_end;
+      stop = STOP_T_END;
+      break;
+    }
+    t = t + delta;
+    for (int32_t k = 0; k < M; ++k) { const double inc = a[k] * delta; T[k] = T[k] + inc; }
+    for (int64_t e = net.stoich_ptr[mu]; e < net.stoich_ptr[mu + 1]; ++e) {
+      int64_t &xj = X[net.stoich_species[e]];
+      xj += net.stoich_v[e];
+      if (xj < 0) rc = ERR_BAD;
+      if (xj > xmax) rc = ERR_OVERFLOW;
+    }
+    n[mu] += 1u;
+    P[mu] = P[mu] + exp_draw(seed, traj, (uint32_t)mu, n[mu]);
+    if (fired < trace_cap) {
+      if (trace_mu) trace_mu[fired] = mu;
+      if (trace_t) trace_t[fired] = t;
+    }
+    fired += 1;
+    if (rc != OK) break;
+    if (max_firings != 0 && fired == max_firings) { stop = STOP_MAX_FIRINGS; break; }
+  }
+  if (x_out) for (int32_t j = 0; j < N; ++j) x_out[j] = X[j];
+  if (t_out) *t_out = t;
+  if (firings_out) *firings_out = fired;
+  if (stop_out) *stop_out = stop;
+  if (fire_count_out) for (int32_t k = 0; k < M; ++k) fire_count_out[k] = n[k];
+  if (T_out) for (int32_t k = 0; k < M; ++k) T_out[k] = T[k];
+  if (P_out) for (int32_t k = 0; k < M; ++k) P_out[k] = P[k];
+  return rc;
+}
+
 }  // namespace
 
 extern "C" {
@@ -309,6 +417,20 @@ int oracle_run(int32_t N, int32_t M, const int64_t *react_ptr, const int32_t *re
   Net net{N, M, react_ptr, react_species, react_sigma, stoich_ptr, stoich_species, stoich_v, rate};
   return nrrta_run(net, x0, seed, traj, max_firings, t_end, x_out, t_out, firings_out,
                    stop_out, fire_count_out, T_out, P_out, trace_mu, trace_t, trace_cap);
+}
+
+int oracle_run_sched(int32_t N, int32_t M, const int64_t *react_ptr, const int32_t *react_species,
+                     const int32_t *react_sigma, const int64_t *stoich_ptr,
+                     const int32_t *stoich_species, const int32_t *stoich_v, const double *rate,
+                     const int64_t *x0, uint64_t seed, uint64_t traj, uint64_t max_firings,
+                     double t_end, int32_t n_break, const double *t_break, const double *factor,
+                     const uint8_t *mask, int64_t *x_out, double *t_out, uint64_t *firings_out,
+                     int32_t *stop_out, uint64_t *fire_count_out, double *T_out, double *P_out,
+                     int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
+  Net net{N, M, react_ptr, react_species, react_sigma, stoich_ptr, stoich_species, stoich_v, rate};
+  return nrrta_run_sched(net, x0, seed, traj, max_firings, t_end, n_break, t_break, factor, mask,
+                         x_out, t_out, firings_out, stop_out, fire_count_out, T_out, P_out,
+                         trace_mu, trace_t, trace_cap);
 }
 
 int oracle_run_residual(int32_t N, int32_t M, const int64_t *react_ptr, const int32_t *react_species,

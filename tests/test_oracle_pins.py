@@ -374,3 +374,66 @@ def test_residual_form_agrees_in_distribution_with_direct_method(case):
     xd, _ = direct_method(net, x0, n_traj, t_end, seed=999)
     for j in range(net["n_species"]):
         _two_sample(xs[:, j].astype(float), xd[:, j].astype(float))
+
+
+# ------------------------------------------------------------------ time-dependent rates (Eq.28)
+def _piecewise_inverse(target, c, t_break, factor):
+    """Smallest t with int_0^t c*f(s) ds = target for piecewise-constant f (f = 1 before
+    t_break[0]); math.inf if the integral never reaches target.  Plain Python floats."""
+    t, acc, f = 0.0, 0.0, 1.0
+    edges = list(t_break) + [math.inf]
+    facs = list(factor)
+    for i, b in enumerate(edges):
+        rate = c * f
+        if rate > 0 and acc + rate * (b - t) >= target:
+            return t + (target - acc) / rate
+        if b == math.inf:
+            return math.inf
+        acc += rate * (b - t)
+        t, f = b, facs[i]
+    return math.inf
+
+
+def test_time_dependent_single_channel_closed_form():
+    """Eq.28 for one source channel with piecewise-constant c(t): the n-th firing
+    time solves int_0^{t_n} c f(s) ds = sum_{i<n} E_i, across several breakpoints, a zero-rate
+    window, and a breakpoint exactly at 0."""
+    c = 3.0
+    net = W.from_reactions(1, [({}, {0: 1}, c)])
+    for t_break, factor in (((0.5, 1.25, 2.0), (4.0, 0.0, 0.5)), ((0.0, 1.0), (2.0, 0.25))):
+        o = oracle.run_sched(net, [0], seed=3, trajectory=8, max_firings=60, trace_cap=60,
+                             t_break=t_break, factor=factor)
+        acc = 0.0
+        for i in range(o["firings"]):
+            acc += oracle.exp_draw(3, 8, 0, i)
+            want = _piecewise_inverse(acc, c, t_break, factor)
+            assert math.isclose(o["trace_t"][i], want, rel_tol=1e-12), (i, o["trace_t"][i], want)
+        assert o["firings"] == 60
+
+
+def test_time_dependent_mask_and_zero_window():
+    """Only masked channels are modulated; while their factor is 0 they never fire, the others go on."""
+    net, x0 = W.birth_death()                      # 0 -> X (c=10), X -> 0 (c=0.1)
+    o = oracle.run_sched(net, [50], seed=5, trajectory=0, t_end=30.0, trace_cap=4000,
+                         t_break=(10.0, 20.0), factor=(0.0, 1.0), mask=[1, 0])
+    tt, mu = o["trace_t"], o["trace_mu"]
+    window = (tt > 10.0) & (tt <= 20.0)
+    assert window.any() and (mu[window] == 1).all()          # only deaths inside the window
+    assert (mu[tt <= 10.0] == 0).any() and (mu[tt > 20.0] == 0).any()
+    assert o["stop"] == oracle.STOP_T_END and o["t"] == 30.0
+    # no schedule at all == the plain oracle, bit for bit
+    a = oracle.run_sched(net, [50], 5, 0, 500, trace_cap=500)
+    b = oracle.run(net, [50], 5, 0, 500, trace_cap=500)
+    np.testing.assert_array_equal(a["trace_mu"], b["trace_mu"])
+    np.testing.assert_array_equal(a["trace_t"], b["trace_t"])
+
+
+def test_time_dependent_birth_count_is_poisson():
+    """Births with rate c f(t): N(t_end) ~ Poisson(int c f) (inhomogeneous Poisson process)."""
+    net = W.from_reactions(1, [({}, {0: 1}, 2.0)])
+    t_break, factor = (1.0, 3.0), (5.0, 0.5)
+    mean = 2.0 * (1.0 + 5.0 * 2.0 + 0.5 * 1.0)                # t_end = 4
+    xs = np.array([oracle.run_sched(net, [0], 17, i, 0, 4.0, t_break=t_break, factor=factor)["x"][0]
+                   for i in range(3000)], dtype=float)
+    assert abs(xs.mean() - mean) < 3 * math.sqrt(mean / xs.size)
+    assert abs(xs.var(ddof=1) - mean) < 3 * mean * math.sqrt(2.0 / (xs.size - 1)) + 3 * math.sqrt(mean / xs.size)
