@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--scale", type=float, default=1.0, help="shrink N, M (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="name=value for rt_set_option")
+    ap.add_argument("--breakpoints", type=int, default=0,
+                    help="time-dependent rates (Eq.28): this many rate breakpoints spread over the step")
     return ap.parse_args()
 
 
@@ -200,6 +202,16 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.breakpoints > 0:
+        # learn how long (in simulated time) a step is, then spread the breakpoints over it:
+        # factors alternate 1.5 / 0.5 on the even-numbered reactions
+        step_dev()
+        torch.cuda.synchronize()
+        t_final = float(res_dev.cpu().numpy().view(rt.RESULT_DTYPE)["t"].max())
+        nb = args.breakpoints
+        tb = [t_final * (i + 1) / (nb + 2) for i in range(nb)]
+        fa = [1.5 if i % 2 == 0 else 0.5 for i in range(nb)]
+        model.set_rate_schedule(tb, fa, (np.arange(M) % 2 == 0).astype(np.uint8))
     for _ in range(max(args.warmup, 3)):
         flush.fill_(1)
         step_dev()
@@ -283,7 +295,8 @@ def run_cuda(args):
                        "state_in_shared_memory": bool(model.info("state_in_smem")),
                        "us_per_firing": 1e6 * kernel_s / fired_per_step * n_traj,
                        "ensemble_path": model.info("ensemble_path"),
-                       "formulation": "residual (Table 3)" if formulation else "(T, P) internal time"},
+                       "formulation": "residual (Table 3)" if formulation else "(T, P) internal time",
+                       "rate_breakpoints": args.breakpoints},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},
             "gpu_launches": int(launches),

@@ -132,6 +132,21 @@ int rt_ensemble_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t 
  * reported a barrier timeout or the runtime reported an error. */
 int rt_sync(rt_model *m, void *stream);
 
+/* Time-dependent rates (section 6, Eq.28, :224-231: channel k fires when
+ * h_k * int_t^{t+dt_k} c_k(s) ds = P_k - T_k, "calculated analytically for well behaved
+ * time-dependent reaction rates").  The family implemented is piecewise-constant modulation:
+ *   c_k(s) = c_k * factor[i]  for s in [t_break[i], t_break[i+1])   (factor 1 before t_break[0])
+ * for the reactions with mask[k] != 0 (mask == NULL: all reactions); the effective rate is the
+ * one rounded product c_k * factor[i].  A step that would cross a breakpoint is cut there
+ * (T_k += a_k * (b - t) for every k, t = b, nothing fires) and the rates switch.
+ *   t_break [n_break] strictly increasing, finite, >= 0;  factor [n_break] finite, >= 0;
+ *   mask [M] or NULL.  n_break = 0 removes the schedule.  The arrays are copied.
+ * Applies to rt_run / rt_ensemble (and their _dev forms) through the bundle kernel; not
+ * combinable with "refresh_mode" = 1 or "formulation" = 1 (RT_ERR_UNSUPPORTED at run time).
+ * Returns RT_ERR_BAD_ARG for an invalid schedule. */
+int rt_set_rate_schedule(rt_model *m, int32_t n_break, const double *t_break, const double *factor,
+                         const uint8_t *mask);
+
 /* Tuning / debug knobs (all optional; results never depend on them, except "formulation").
  *   "refresh_mode"   0 = dependency-graph refresh of a_k (default), 1 = recompute every a_k
  *                    each firing (the paper's own GPU scheme)

@@ -58,13 +58,14 @@ def lib():
     L.rt_ensemble.argtypes = [vp, vp, u64, u64, u64, u64, f64, vp, vp]
     L.rt_ensemble_dev.argtypes = [vp, vp, u64, u64, u64, u64, f64, vp, vp, vp]
     L.rt_sync.argtypes = [vp, vp]
+    L.rt_set_rate_schedule.argtypes = [vp, C.c_int32, vp, vp, vp]
     L.rt_set_option.argtypes = [vp, C.c_char_p, i64]
     L.rt_get_info.argtypes = [vp, C.c_char_p, C.POINTER(i64)]
     L.rt_destroy.argtypes = [vp]
     L.rt_destroy.restype = None
     L.rt_strerror.argtypes = [i32]
     L.rt_strerror.restype = C.c_char_p
-    for name in ("rt_validate_network", "rt_create", "rt_run", "rt_run_dev", "rt_ensemble",
+    for name in ("rt_validate_network", "rt_create", "rt_run", "rt_run_dev", "rt_ensemble", "rt_set_rate_schedule",
                  "rt_ensemble_dev", "rt_sync", "rt_set_option", "rt_get_info"):
         getattr(L, name).restype = i32
     _lib = L
@@ -108,6 +109,17 @@ def rt_create(net, device=0):
 def rt_destroy(handle):
     if handle:
         lib().rt_destroy(C.c_void_p(handle))
+
+
+def rt_set_rate_schedule(handle, t_break, factor, mask=None):
+    """Piecewise-constant rate modulation (include/rt.h); empty t_break removes it."""
+    tb = _np(t_break, np.float64)
+    fa = _np(factor, np.float64)
+    if tb.shape != fa.shape or tb.ndim != 1:
+        return RT_ERR_BAD_ARG
+    mk = None if mask is None else _np(mask, np.uint8)
+    return lib().rt_set_rate_schedule(C.c_void_p(handle), int(tb.size), _ptr(tb) if tb.size else None,
+                                      _ptr(fa) if fa.size else None, _ptr(mk))
 
 
 def rt_set_option(handle, name, value):
@@ -211,6 +223,11 @@ class Model:
         rc = rt_set_option(self.handle, name, value)
         if rc != RT_OK:
             raise RtError(rc, f"rt_set_option({name})")
+
+    def set_rate_schedule(self, t_break, factor, mask=None):
+        rc = rt_set_rate_schedule(self.handle, t_break, factor, mask)
+        if rc != RT_OK:
+            raise RtError(rc, "rt_set_rate_schedule")
 
     def info(self, name):
         return rt_get_info(self.handle, name)

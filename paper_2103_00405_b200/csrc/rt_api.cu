@@ -69,6 +69,10 @@ struct rt_model {
       d_rate, d_srow, d_sp_rec, d_sp_big, d_big_off, d_dep;
   // per-bundle state
   DevBuf d_T, d_P, d_a, d_n, d_X, d_exch, d_err;
+  // rate schedule (time-dependent rates)
+  DevBuf d_sched_t, d_sched_f, d_sched_mask;
+  int sched_n = 0;
+  bool sched_has_mask = false;
   // staging for the host-pointer API
   DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t;
   // options
@@ -211,14 +215,22 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.refresh_mode = m->refresh_mode;
   p.prefetch = m->opt_prefetch;
   p.formulation = m->opt_formulation;
+  if (m->sched_n > 0 && (m->refresh_mode != 0 || m->opt_formulation != 0)) return RT_ERR_UNSUPPORTED;
+  p.sched_n = m->sched_n;
+  p.sched_t = (const double *)m->d_sched_t.p;
+  p.sched_f = (const double *)m->d_sched_f.p;
+  p.sched_mask = m->sched_has_mask ? (const unsigned char *)m->d_sched_mask.p : nullptr;
   p.err = (int *)m->d_err.p;
   void *args[] = {&p};
   // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
   const void *kern;
-  if (pl.smem) kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlock, true, true>
-                                      : (const void *)rt::rt_bundle_kernel<kBlock, true, false>;
-  else kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlock, false, true>
-                              : (const void *)rt::rt_bundle_kernel<kBlock, false, false>;
+  const bool sched = m->sched_n > 0;       // (never together with refresh_mode 1: checked above)
+  if (pl.smem) kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlock, true, true, false>
+                      : sched         ? (const void *)rt::rt_bundle_kernel<kBlock, true, false, true>
+                                      : (const void *)rt::rt_bundle_kernel<kBlock, true, false, false>;
+  else kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlock, false, true, false>
+              : sched         ? (const void *)rt::rt_bundle_kernel<kBlock, false, false, true>
+                              : (const void *)rt::rt_bundle_kernel<kBlock, false, false, false>;
   const size_t dyn = pl.smem ? smem_state_bytes(pl.pairs_per_cta) : 0;
   if (dyn) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
   // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
@@ -476,7 +488,8 @@ int rt_ensemble_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t 
   if (rc != RT_OK) return rc;
   if (n_traj == 0) return RT_OK;
   CU_TRY(cudaSetDevice(m->device));
-  bool use_threads = thread_path_fits(m) && m->opt_formulation == 0;   // (the thread kernel is (T,P) only)
+  // (the thread kernel implements the plain (T,P) form with constant rates only)
+  bool use_threads = thread_path_fits(m) && m->opt_formulation == 0 && m->sched_n == 0;
   if (m->opt_ensemble_path == 1) {
     if (!thread_path_fits(m)) return RT_ERR_BAD_ARG;
     use_threads = true;
@@ -521,6 +534,27 @@ int rt_sync(rt_model *m, void *stream) {
   if (!m) return RT_ERR_NULL;
   CU_TRY(cudaSetDevice(m->device));
   return finish(m, (cudaStream_t)stream);
+}
+
+int rt_set_rate_schedule(rt_model *m, int32_t n_break, const double *t_break, const double *factor,
+                         const uint8_t *mask) {
+  if (!m) return RT_ERR_NULL;
+  if (n_break < 0 || n_break > (1 << 20)) return RT_ERR_BAD_ARG;
+  if (n_break == 0) { m->sched_n = 0; m->sched_has_mask = false; return RT_OK; }
+  if (!t_break || !factor) return RT_ERR_NULL;
+  for (int32_t i = 0; i < n_break; ++i) {
+    if (!std::isfinite(t_break[i]) || t_break[i] < 0.0 || !std::isfinite(factor[i]) || factor[i] < 0.0)
+      return RT_ERR_BAD_ARG;
+    if (i > 0 && !(t_break[i] > t_break[i - 1])) return RT_ERR_BAD_ARG;
+  }
+  CU_TRY(cudaSetDevice(m->device));
+  int rc;
+  if ((rc = upload(m->d_sched_t, std::vector<double>(t_break, t_break + n_break))) != RT_OK) return rc;
+  if ((rc = upload(m->d_sched_f, std::vector<double>(factor, factor + n_break))) != RT_OK) return rc;
+  m->sched_has_mask = mask != nullptr;
+  if (mask && (rc = upload(m->d_sched_mask, std::vector<uint8_t>(mask, mask + m->net.M))) != RT_OK) return rc;
+  m->sched_n = n_break;
+  return RT_OK;
 }
 
 int rt_set_option(rt_model *m, const char *name, int64_t value) {
@@ -575,7 +609,8 @@ void rt_destroy(rt_model *m) {
                     &m->d_stoich_species, &m->d_stoich_v, &m->d_rate, &m->d_srow,
                     &m->d_sp_rec, &m->d_sp_big, &m->d_big_off, &m->d_dep,
                     &m->d_T, &m->d_P, &m->d_a, &m->d_n, &m->d_X, &m->d_exch, &m->d_err,
-                    &m->d_x0, &m->d_xout, &m->d_res, &m->d_trace_mu, &m->d_trace_t};
+                    &m->d_x0, &m->d_xout, &m->d_res, &m->d_trace_mu, &m->d_trace_t,
+                    &m->d_sched_t, &m->d_sched_f, &m->d_sched_mask};
   for (DevBuf *b : bufs) b->release();
   delete m;
 }

@@ -62,6 +62,11 @@ struct BundleParams {
   int formulation;        // 0: (T, P) internal-time form; 1: residual (Table 3) form, kept as
                           //    T_k = -R_k with P_k = 0 (same operations, one array less to read)
   int refresh_mode;       // 0 dependency walk, 1 recompute every a_k (the paper's GPU scheme)
+  // time-dependent rates (Eq.28, piecewise constant): c_k(t) = c_k * sched_f[i] for t in
+  // [sched_t[i], sched_t[i+1]) for the channels with sched_mask[k] != 0 (all if nullptr)
+  int sched_n;
+  const double *sched_t, *sched_f;
+  const unsigned char *sched_mask;
   int *err;               // set to 1 on a barrier timeout
 };
 
@@ -350,10 +355,22 @@ __device__ __forceinline__ DepEnt load_dep(const NetDev &net, uint32_t idx) {
   return e;
 }
 
+// Effective rate constant of reaction k under the rate schedule: one rounded product c_k * f.
+template <bool SCHED>
+__device__ __forceinline__ double eff_rate(const BundleParams &p, int k, double c, double fac) {
+  if (SCHED && (p.sched_mask == nullptr || __ldg(p.sched_mask + k))) return __dmul_rn(c, fac);
+  return c;
+}
+__device__ __forceinline__ double propensity_eff(const BundleParams &p, const u64 *X, int k, double fac) {
+  return propensity_csr(eff_rate<true>(p, k, __ldg(p.net.rate + k), fac), p.net.react_ptr, p.net.react_species,
+                        p.net.react_sigma, X, k);
+}
+
 // New propensity of the reaction of entry d = (k, j1, j2, sigma1 | sigma2 << 8 | general << 16)
 // with rate c: same operation order as propensity().
 __device__ __forceinline__ double propensity_dep(const NetDev &net, const u64 *X, const int4 d, double c) {
-  if (d.w & 0x10000) return propensity(net, X, d.x);    // more than two reactants (rare)
+  if (d.w & 0x10000)                                    // more than two reactants (rare)
+    return propensity_csr(c, net.react_ptr, net.react_species, net.react_sigma, X, d.x);
   const long long x1 = x_load(X, d.y);
   const long long x2 = x_load(X, d.z >= 0 ? d.z : d.y);
   double a = __dmul_rn(c, __ll2double_rn(binom(x1, d.w & 0xff)));
@@ -404,13 +421,14 @@ __device__ __forceinline__ bool walk_scan(const NetDev &net, const Ranges &rg, u
 }
 
 // Finish: new a_k for the n compacted entries (X loads of 32 entries in flight together).
-__device__ __forceinline__ void walk_finish(const NetDev &net, const u64 *X, int lane, int n,
-                                            const int4 *list_d, int *list_k, double *list_a) {
+template <bool SCHED>
+__device__ __forceinline__ void walk_finish(const BundleParams &p, double fac, const u64 *X, int lane,
+                                            int n, const int4 *list_d, int *list_k, double *list_a) {
   __syncwarp();
   for (int i = lane; i < n; i += 32) {
     const int4 d = list_d[i];
     list_k[i] = d.x;
-    list_a[i] = propensity_dep(net, X, d, list_a[i]);
+    list_a[i] = propensity_dep(p.net, X, d, eff_rate<SCHED>(p, d.x, list_a[i], fac));
   }
 }
 
@@ -623,7 +641,8 @@ __device__ __noinline__ bool bundle_barrier(u64 *exch, int S, int r, uint32_t ge
 
 // FULL = refresh_mode 1 (recompute every a_k each firing, the paper's own GPU scheme) is a separate
 // instantiation so that its code stays out of the instruction stream of the default kernel.
-template <int BLOCK, bool SMEM, bool FULL>
+// SCHED = a rate schedule is set (time-dependent rates): also its own instantiation.
+template <int BLOCK, bool SMEM, bool FULL, bool SCHED>
 __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams p) {
   constexpr int NT = BLOCK - 32 * kWalkerWarps;      // stream threads; the last warp walks
   __shared__ BundleCtx<BLOCK> ctx;
@@ -703,6 +722,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     u64 fired = 0;
     int mu_prev = -1, stop = 0, status = RT_OK;
     bool finishing = false;
+    double fac = 1.0, fac_next = 1.0;   // rate schedule: current factor, factor after the breakpoint
+    int seg = 0;                        //   breakpoints passed
+    bool rate_change = false;           //   this pass ends at a breakpoint: recompute every a_k
     constexpr bool full = FULL;
 
     for (;;) {   // one iteration per firing, plus one closing pass
@@ -773,16 +795,18 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           }
           __syncwarp();
           if (has0) {
+            c0 = eff_rate<SCHED>(p, d0.x, c0, fac);
             double a = __dmul_rn(c0, __ll2double_rn(binom(x1, d0.w & 0xff)));
             if (d0.z >= 0) a = __dmul_rn(a, __ll2double_rn(binom(x2, (d0.w >> 8) & 0xff)));
-            if (d0.w & 0x10000) a = propensity(net, X, d0.x);       // > 2 reactants: after the update
+            if (d0.w & 0x10000)                                     // > 2 reactants: after the update
+              a = propensity_csr(c0, net.react_ptr, net.react_species, net.react_sigma, X, d0.x);
             list_k[lane] = d0.x;
             list_a[lane] = a;
           }
           for (int i = lane + 32; i < spec.pw_n; i += 32) {        // more than 32: plain path
             const int4 d = pw_d[i];
             list_k[i] = d.x;
-            list_a[i] = propensity_dep(net, X, d, pw_c[i]);
+            list_a[i] = propensity_dep(net, X, d, eff_rate<SCHED>(p, d.x, pw_c[i], fac));
           }
           pre_n = spec.pw_n;
         } else if (!w_csr) {
@@ -880,7 +904,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
               w_f = 0;
             }
           }
-          if (pre_n < 0) walk_finish(net, X, lane, n, list_d, list_k, list_a);
+          if (pre_n < 0) walk_finish<SCHED>(p, fac, X, lane, n, list_d, list_k, list_a);
           if (lane == 0) { ctx.list_n = n; ctx.more = more ? 1 : 0; }
         } else if (first_round) {
           // ===== stream warps: a-5 of the previous firing fused with a-2/a-3 of this one =====
@@ -933,7 +957,24 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         first_round = false;
       }
       PT_MARK(2)
-      if (SMEM) {
+      if (SCHED && rate_change) {
+        // the pass above brought every T_k to the breakpoint with the old rates; now switch
+        rate_change = false;
+        fac = fac_next;
+        for (int k = k0 + tid; k < k1; k += BLOCK)
+          if (k < M) {
+            const double a_new = propensity_eff(p, X, k, fac);
+            if (SMEM) sA[k - k0] = a_new; else __stcg(A + k, a_new);
+            if (filter_unsafe(a_new)) ctx.any_odd = 1;
+          }
+        dirty[tid] = 0;
+        __syncthreads();
+        if (!is_walker) {
+          bool defer = false;
+          best = scan_own<NT, SMEM, false>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, 0.0, false, cnt_pad,
+                                           ctx.any_odd != 0, defer, resid);
+        }
+      } else if (SMEM) {
         // re-scan (read-only) with the new a_k, P_mu.  Stale threads are few (usually one, in the
         // CTA that owns the fired reaction, which is then the last to post), so the thread's warp
         // shares its reactions: one exact division per lane instead of a serial pass.
@@ -997,6 +1038,20 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
 
       // ---- a-4 stop tests, identical in every thread of every CTA of the bundle
       const double delta = win.dt;
+      if (SCHED) {
+        // Eq.28 with piecewise-constant c_k(t): a step that would cross the next breakpoint is cut
+        // there -- T_k += a_k (b - t), t = b, no firing -- and the rates switch.
+        const double tb = (seg < p.sched_n && __ldg(p.sched_t + seg) <= p.t_end) ? __ldg(p.sched_t + seg) : INF;
+        if (tb < INF && (delta == INF || __dadd_rn(t, delta) > tb)) {
+          dprev = __dsub_rn(tb, t);
+          t = tb;
+          mu_prev = -1;
+          fac_next = __ldg(p.sched_f + seg);
+          seg += 1;
+          rate_change = true;
+          continue;
+        }
+      }
       if (delta == INF) { stop = RT_STOP_ABSORBED; break; }
       if (p.t_end < INF && __dadd_rn(t, delta) > p.t_end) {
         dprev = __dsub_rn(p.t_end, t);           // closing pass: T_k += a_k * (t_end - t), no firing

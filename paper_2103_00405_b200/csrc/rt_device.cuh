@@ -99,10 +99,10 @@ __device__ __forceinline__ long long x_load(const u64 *Xv, int j) { return x_cou
 // a_k = c_k * prod_j C(X_j, sigma_jk): one rounded multiply per reactant, CSR order.
 // X is read with ld.global.cg (L2): other CTAs write it too.  Not inlined (code size); takes the
 // arrays rather than the NetDev so that no copy of the kernel parameters is forced into local memory.
-__device__ __noinline__ double propensity_csr(const double *rate, const uint32_t *react_ptr,
+__device__ __noinline__ double propensity_csr(double c, const uint32_t *react_ptr,
                                               const int32_t *react_species, const int32_t *react_sigma,
                                               const u64 *Xv, int k) {
-  double a = __ldg(rate + k);
+  double a = c;
   const uint32_t e1 = __ldg(react_ptr + k + 1);
   for (uint32_t e = __ldg(react_ptr + k); e < e1; ++e) {
     const long long x = x_load(Xv, __ldg(react_species + e));
@@ -111,7 +111,7 @@ __device__ __noinline__ double propensity_csr(const double *rate, const uint32_t
   return a;
 }
 __device__ __forceinline__ double propensity(const NetDev &net, const u64 *Xv, int k) {
-  return propensity_csr(net.rate, net.react_ptr, net.react_species, net.react_sigma, Xv, k);
+  return propensity_csr(__ldg(net.rate + k), net.react_ptr, net.react_species, net.react_sigma, Xv, k);
 }
 
 // ------------------------------------------------------------------ lexicographic argmin

@@ -366,3 +366,73 @@ def test_residual_form_cfg4_prefix_and_differs_from_default(rt):
     with rt.Model(net) as m:
         d = m.run(x0, par["seed"], 0, 1500, trace_cap=1500)
     assert d["trace_mu"][0] == g["trace_mu"][0]          # same first draws -> same first firing
+
+
+# ------------------------------------------------------------------ time-dependent rates (Eq.28)
+def _check_sched(rt, net, x0, seed, traj, max_firings, t_end, trace_cap, t_break, factor, mask,
+                 options=()):
+    o = _oracle().run_sched(net, x0, seed, traj, max_firings, t_end, trace_cap,
+                            t_break=t_break, factor=factor, mask=mask)
+    with rt.Model(net) as m:
+        for name, val in options:
+            m.set_option(name, val)
+        m.set_rate_schedule(t_break, factor, mask)
+        g = m.run(x0, seed, traj, max_firings, t_end, trace_cap, want_state=True)
+    assert g["firings"] == o["firings"] and g["stop"] == o["stop"]
+    np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["fire_count"], o["fire_count"])
+    np.testing.assert_allclose(g["trace_t"], o["trace_t"], rtol=RTOL_T, atol=0)
+    assert math.isclose(g["t"], o["t"], rel_tol=RTOL_T, abs_tol=0)
+    np.testing.assert_allclose(g["T"], o["T"], rtol=1e-10, atol=1e-12)
+    np.testing.assert_allclose(g["P"], o["P"], rtol=1e-12, atol=0)
+    return g, o
+
+
+@pytest.mark.parametrize("ctas,state_mode", [(0, 0), (3, 0), (1, 1), (0, 1)])
+def test_time_dependent_rates_match_oracle(rt, ctas, state_mode):
+    """PAPER.md Eq.28 with piecewise-constant c_k(t): several breakpoints inside the run (the
+    network fires ~2e5 times per unit time, so they fall between firings), a zero-rate window
+    for a masked half of the reactions, with the state in shared and in global memory."""
+    net, x0, par = W.make_config("cfg3", scale=0.03)
+    M = int(net["n_reactions"])
+    mask = (np.arange(M) % 2).astype(np.uint8)
+    o0 = _oracle().run(net, x0, par["seed"], 1, 1200, math.inf, 1200)
+    tt = o0["trace_t"]
+    t_break = [float(tt[150]) * 1.0000001, float(tt[400]), float(tt[800]) * 0.9999999]
+    factor = [3.0, 0.0, 0.5]
+    opts = [("bundle_ctas", ctas), ("state_mode", state_mode)]
+    _check_sched(rt, net, x0, par["seed"], 1, 1500, math.inf, 1500, t_break, factor, mask, opts)
+    _check_sched(rt, net, x0, par["seed"], 1, 1500, math.inf, 1500, t_break, factor, None, opts)
+    # a t_end between two breakpoints: later breakpoints must not act
+    g, o = _check_sched(rt, net, x0, par["seed"], 1, 0, float(tt[600]), 4096, t_break, factor, mask, opts)
+    assert g["stop"] == rt.RT_STOP_T_END
+
+
+def test_time_dependent_rates_revive_an_absorbed_state(rt):
+    """All rates 0 until the first breakpoint: nothing can fire, the run must jump to the
+    breakpoint instead of reporting ABSORBED, then proceed; hub network (pre-walk, staging rounds)."""
+    net, x0 = _hub_network()
+    o0 = _oracle().run(net, x0, 21, 0, 300, math.inf, 300)
+    b1 = float(o0["trace_t"][100])
+    _check_sched(rt, net, x0, 21, 0, 500, math.inf, 500, [0.0, b1, 2 * b1], [0.0, 1.0, 2.5], None)
+
+
+def test_rate_schedule_validation_and_unsupported_combinations(rt):
+    net, x0 = W.lotka_volterra()
+    with rt.Model(net) as m:
+        assert rt.rt_set_rate_schedule(m.handle, [1.0, 0.5], [1.0, 1.0]) == rt.RT_ERR_BAD_ARG   # not increasing
+        assert rt.rt_set_rate_schedule(m.handle, [-1.0], [1.0]) == rt.RT_ERR_BAD_ARG
+        assert rt.rt_set_rate_schedule(m.handle, [1.0], [-2.0]) == rt.RT_ERR_BAD_ARG
+        assert rt.rt_set_rate_schedule(m.handle, [1.0], [math.inf]) == rt.RT_ERR_BAD_ARG
+        m.set_rate_schedule([0.01], [2.0])
+        m.set_option("refresh_mode", 1)
+        assert m.run(x0, 1, 0, 10, check=False)["code"] == rt.RT_ERR_UNSUPPORTED
+        m.set_option("refresh_mode", 0)
+        ens = m.ensemble(x0, 2, 0, 5, 300, math.inf)          # tiny network, schedule -> bundle path
+        assert m.info("ensemble_path") == 2
+        o = [_oracle().run_sched(net, x0, 2, i, 300, math.inf, 0, t_break=[0.01], factor=[2.0])["x"] for i in range(5)]
+        np.testing.assert_array_equal(ens["x"], np.array(o))
+        m.set_rate_schedule([], [])                            # removed again
+        a = m.run(x0, 2, 0, 300)
+        np.testing.assert_array_equal(a["x"], _oracle().run(net, x0, 2, 0, 300)["x"])
