@@ -477,12 +477,11 @@ struct Spec {
 template <int BLOCK, bool PREWALK>
 __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<BLOCK> &ctx,
                                               u64 *exch, const uint32_t *nfire, int r,
-                                              uint32_t &gen, Cand mine, bool fence, Spec &spec) {
+                                              uint32_t &gen, Cand mine, Spec &spec) {
   constexpr int NT = BLOCK - 32 * kWalkerWarps;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   mine = warp_lexmin(mine);
   if (lane == 0) ctx.warp_part[warp] = mine;
-  if (fence) __threadfence();
   __syncthreads();
   if (warp == 0) {
     Cand c = ctx.warp_part[lane];                 // BLOCK / 32 <= 32 partials
@@ -535,7 +534,7 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
       if (timed_out) c.k = -2;
     }
     if (lane == 0) { ctx.win = c; ctx.second_k = (c2.dt < __longlong_as_double(0x7ff0000000000000ll)) ? c2.k : 0x7fffffff; }
-  } else if (warp == BLOCK / 32 - 1 && !fence) {
+  } else if (warp == BLOCK / 32 - 1) {
     // Walker warp, idle during the exchange.  If this CTA's candidate wins (it usually stays the
     // candidate for many firings before it does), this CTA must redraw P_k (Philox + log, the
     // longest serial piece of a firing) and every CTA will need the candidate's stoich row and
@@ -595,16 +594,11 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
     }
   }
   gen += 1u;
-  if (fence) {
-    __syncthreads();
-    __threadfence();
-  } else {
-    // The stream warps leave as soon as warp 0 has the winner; the walker warp, which may still
-    // be busy with its speculative work, pairs with warp 0 on a barrier of its own.
-    if (warp == 0) asm volatile("bar.arrive 2, 64;" ::: "memory");
-    if (warp == BLOCK / 32 - 1) { asm volatile("bar.sync 2, 64;" ::: "memory"); spec.k2 = ctx.second_k; }
-    else asm volatile("bar.sync 1, %0;" ::"r"(NT) : "memory");
-  }
+  // The stream warps leave as soon as warp 0 has the winner; the walker warp, which may still
+  // be busy with its speculative work, pairs with warp 0 on a barrier of its own.
+  if (warp == 0) asm volatile("bar.arrive 2, 64;" ::: "memory");
+  if (warp == BLOCK / 32 - 1) { asm volatile("bar.sync 2, 64;" ::: "memory"); spec.k2 = ctx.second_k; }
+  else asm volatile("bar.sync 1, %0;" ::"r"(NT) : "memory");
   return ctx.win;
 }
 
@@ -1032,7 +1026,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
 
       // ---- a-3 argmin over the bundle
       PT_MARK(3)
-      const Cand win = bundle_argmin<BLOCK, SMEM>(p, ctx, exch, nfire, r, gen, best, false, spec);
+      const Cand win = bundle_argmin<BLOCK, SMEM>(p, ctx, exch, nfire, r, gen, best, spec);
       PT_MARK(4)
       if (win.k == -2) return;
 
