@@ -78,7 +78,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
-                 "--format=csv,noheader,nounits", "-lms", "100"],
+                 "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -305,7 +305,11 @@ def run_cuda(args):
                          "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
                          "kernel": "rt_bundle_kernel", "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": alg_bytes,
-                         "frac_of_8TBs_nominal": achieved / 8000.0},
+                         "frac_of_8TBs_nominal": achieved / 8000.0,
+                         "note": ("state (T,P,a) resident in shared memory: `achieved` is algorithmic "
+                                  "bytes per second, not DRAM throughput (see `traffic`); the step is "
+                                  "latency-bound (DESIGN.md 7)") if model.info("state_in_smem")
+                         else "state streamed from global memory: DRAM traffic = algorithmic bytes"},
         }
         if args.workload in THREAD_INSTR_PER_STEP:
             # one thread per trajectory, state in shared memory: plain ALU issue is the bound
