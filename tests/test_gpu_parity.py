@@ -436,3 +436,25 @@ def test_rate_schedule_validation_and_unsupported_combinations(rt):
         m.set_rate_schedule([], [])                            # removed again
         a = m.run(x0, 2, 0, 300)
         np.testing.assert_array_equal(a["x"], _oracle().run(net, x0, 2, 0, 300)["x"])
+
+
+def test_global_state_odd_M_and_ensembles(rt):
+    """State in global memory with an odd number of reactions (one padding slot in the last
+    16-byte pair), for single runs in both formulations and for a multi-bundle ensemble."""
+    net, x0 = _hub_network(n_species=30, n_reactions=4999, seed=9)
+    assert net["n_reactions"] % 2 == 1
+    for ctas in (1, 4):
+        _check_run(rt, net, x0, 13, 0, 400, math.inf, 400,
+                   options=[("state_mode", 1), ("bundle_ctas", ctas)])
+        _check_residual(rt, net, x0, 13, 0, 400, math.inf, 400,
+                        options=[("state_mode", 1), ("bundle_ctas", ctas)])
+    n = 7
+    o = _oracle().ensemble(net, x0, 13, 3, n, 300, math.inf)
+    with rt.Model(net) as m:
+        m.set_option("state_mode", 1)
+        m.set_option("bundle_ctas", 2)
+        g = m.ensemble(x0, 13, 3, n, 300, math.inf)
+        assert m.info("ensemble_path") == 2 and m.info("state_in_smem") == 0 and m.info("bundles") >= 2
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["firings"], o["firings"])
+    np.testing.assert_allclose(g["t"], o["t"], rtol=RTOL_T)
