@@ -20,6 +20,9 @@
  * output buffer; the library copies what it needs during the call and keeps no caller pointer.
  * Results depend only on (network, x0, seed, trajectory, limits) -- not on the launch shape,
  * on how an ensemble is batched, nor on the propensity refresh mode.
+ * A model is not thread-safe: calls on one rt_model must not overlap (different models may).
+ * Device-pointer entry points do not validate device data: x0_dev must hold counts in
+ * [0, bound] (see below), as the host entry points check for x0.
  */
 #ifndef RT_B200_H_
 #define RT_B200_H_
