@@ -13,3 +13,4 @@ from .binding import (  # noqa: F401
     rt_set_option, rt_set_rate_schedule, rt_get_info, rt_destroy, rt_strerror,
 )
 from .dist import shard_range, ensemble_sharded  # noqa: F401
+from .model_file import parse_model, load_model, ModelFileError  # noqa: F401
