@@ -144,6 +144,9 @@ int rt_sync(rt_model *m, void *stream);
  * (T_k += a_k * (b - t) for every k, t = b, nothing fires) and the rates switch.
  *   t_break [n_break] strictly increasing, finite, >= 0;  factor [n_break] finite, >= 0;
  *   mask [M] or NULL.  n_break = 0 removes the schedule.  The arrays are copied.
+ * A factor-0 schedule from t_break[0] = 0 on a mask gives the boundary conditions of the note
+ * under PAPER.md Table 2 (:260): the masked channels are forbidden and their internal time is
+ * frozen.
  * Applies to rt_run / rt_ensemble (and their _dev forms) through the bundle kernel; not
  * combinable with "refresh_mode" = 1 or "formulation" = 1 (RT_ERR_UNSUPPORTED at run time).
  * Returns RT_ERR_BAD_ARG for an invalid schedule. */

@@ -486,3 +486,17 @@ def test_cfg3_scaled_ensemble_beyond_the_bit_exact_horizon(rt):
     ps.append(p)
     for rank, p in enumerate(sorted(ps)):
         assert p > 0.01 / (len(ps) - rank), (rank, p)      # Holm step-down
+
+
+def test_frozen_channels_boundary_condition(rt):
+    """PAPER.md Table 2, note (:260): "the boundary conditions can be achieved by restrict the
+    firing channels.  Those channels that are forbidden for firing is assigned a frozen internal
+    time."  A factor-0 schedule from t = 0 on a mask does exactly that: the masked channels never
+    fire and their internal time T_k stays frozen at 0, the others run as in the oracle."""
+    net, x0, par = W.make_config("cfg3", scale=0.02)
+    M = int(net["n_reactions"])
+    mask = (np.arange(M) % 3 == 0).astype(np.uint8)
+    g, o = _check_sched(rt, net, x0, par["seed"], 0, 1500, math.inf, 1500, [0.0], [0.0], mask)
+    frozen = mask.astype(bool)
+    assert not g["fire_count"][frozen].any() and not g["T"][frozen].any()
+    assert g["fire_count"][~frozen].sum() == 1500 and g["T"][~frozen].any()
