@@ -18,12 +18,21 @@
 
 using rt::u64;
 
-#ifndef RT_BLOCK
-#define RT_BLOCK 512
+#ifndef RT_BLOCK_SMEM
+#define RT_BLOCK_SMEM 256
+#endif
+#ifndef RT_BLOCK_GLOBAL
+#define RT_BLOCK_GLOBAL 512
 #endif
 namespace {
 
-constexpr int kBlock = RT_BLOCK;          // threads per CTA of the bundle kernel (stream warps + 1 walker warp)
+// Threads per CTA of the bundle kernel (stream warps + 1 walker warp).  Measured on B200: with
+// the state in shared memory the pass is issue-bound and every extra warp only lengthens the
+// barriers and the block argmin (cfg4: 256 threads 4.47 us, 384: 4.49, 512: 4.70, 192: 5.35);
+// with the state streamed from HBM more threads keep more bytes in flight (cfg5a: 512 threads
+// 55.7 us, 384: 58.2, 256: 65.4).
+constexpr int kBlockSmem = RT_BLOCK_SMEM;
+constexpr int kBlockGlobal = RT_BLOCK_GLOBAL;
 constexpr int kThreadKernelMaxM = 64; // one-thread-per-trajectory path: M, N at most this
 constexpr int kMinPairsPerCta = 256;  // do not spread a trajectory thinner than this
 constexpr int kBigDeg = 64;           // species read by more reactions than this get a block-offset table
@@ -79,7 +88,7 @@ struct rt_model {
   int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0, opt_prefetch = 7, opt_formulation = 0;
   // info
   int64_t kernel_launches = 0;
-  int last_S = 0, last_B = 0, last_path = 0, last_state_smem = 0;
+  int last_S = 0, last_B = 0, last_path = 0, last_state_smem = 0, last_block = 0;
   size_t n_big = 0;
 };
 
@@ -146,7 +155,7 @@ struct Plan { int S, B, G; int pairs_per_cta; int cnt_pad; bool smem; };
 
 // slots per shared-memory state array: a CTA's reactions padded to whole scan batches
 int padded_count(int pairs_per_cta) {
-  const int batch = rt::kScanBatch * (kBlock - 32 * rt::kWalkerWarps);
+  const int batch = rt::kScanBatch * (kBlockSmem - 32 * rt::kWalkerWarps);
   return (2 * pairs_per_cta + batch - 1) / batch * batch;
 }
 size_t smem_state_bytes(int pairs_per_cta) { return (size_t)padded_count(pairs_per_cta) * 3 * sizeof(double); }
@@ -155,7 +164,7 @@ Plan plan_bundles(const rt_model *m, u64 n_traj) {
   const int pairs_total = m->net.M_pad / 2;
   const int sms = m->num_sms;
   // fewest CTAs whose share of the state still fits in shared memory
-  const int batch = rt::kScanBatch * (kBlock - 32 * rt::kWalkerWarps);
+  const int batch = rt::kScanBatch * (kBlockSmem - 32 * rt::kWalkerWarps);
   const int pairs_fit = std::max(1, (int)(kSmemStateBytes / (3 * sizeof(double)) / batch * batch / 2));
   const int s_fit = (pairs_total + pairs_fit - 1) / pairs_fit;
   const int s_thin = std::max(1, (pairs_total + kMinPairsPerCta - 1) / kMinPairsPerCta);
@@ -225,16 +234,18 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
   const void *kern;
   const bool sched = m->sched_n > 0;       // (never together with refresh_mode 1: checked above)
-  if (pl.smem) kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlock, true, true, false>
-                      : sched         ? (const void *)rt::rt_bundle_kernel<kBlock, true, false, true>
-                                      : (const void *)rt::rt_bundle_kernel<kBlock, true, false, false>;
-  else kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlock, false, true, false>
-              : sched         ? (const void *)rt::rt_bundle_kernel<kBlock, false, false, true>
-                              : (const void *)rt::rt_bundle_kernel<kBlock, false, false, false>;
+  if (pl.smem) kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlockSmem, true, true, false>
+                      : sched         ? (const void *)rt::rt_bundle_kernel<kBlockSmem, true, false, true>
+                                      : (const void *)rt::rt_bundle_kernel<kBlockSmem, true, false, false>;
+  else kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, true, false>
+              : sched         ? (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, false, true>
+                              : (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, false, false>;
   const size_t dyn = pl.smem ? smem_state_bytes(pl.pairs_per_cta) : 0;
   if (dyn) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
   // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
-  CU_TRY(cudaLaunchCooperativeKernel(kern, dim3(pl.S * pl.B), dim3(kBlock), args, dyn, st));
+  const int block = pl.smem ? kBlockSmem : kBlockGlobal;
+  CU_TRY(cudaLaunchCooperativeKernel(kern, dim3(pl.S * pl.B), dim3(block), args, dyn, st));
+  m->last_block = block;
   m->kernel_launches += 1;
   m->last_S = pl.S; m->last_B = pl.B; m->last_path = 2; m->last_state_smem = pl.smem ? 1 : 0;
   return RT_OK;
@@ -591,7 +602,7 @@ int rt_get_info(const rt_model *m, const char *name, int64_t *value) {
   if (!strcmp(name, "kernel_launches")) *value = m->kernel_launches;
   else if (!strcmp(name, "bundle_ctas")) *value = m->last_S;
   else if (!strcmp(name, "bundles")) *value = m->last_B;
-  else if (!strcmp(name, "block_threads")) *value = kBlock;
+  else if (!strcmp(name, "block_threads")) *value = m->last_block;
   else if (!strcmp(name, "ensemble_path")) *value = m->last_path;
   else if (!strcmp(name, "num_sms")) *value = m->num_sms;
   else if (!strcmp(name, "dep_entries")) *value = m->nnz_r;
