@@ -32,9 +32,9 @@ METRIC = "reaction firings/sec on 1 B200 at M=10^6 (+ % of HBM roofline per firi
 UNIT = "firings/s"
 BYTES_PER_REACTION_FIRING = 32   # read T, P, a; write T
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the bundle kernel, from the
-# `ncu --set full` capture of this command (profiles/r1_v6_bundle_kernel.md): 51.47 MB + 2.80 MB.
+# `ncu --set full` capture of this command (profiles/r1_v7_bundle_kernel.md): 51.56 MB + 2.73 MB.
 # Far BELOW the algorithmic bytes: at M = 1e6 the (T,P,a) state lives in shared memory.
-NCU_TRAFFIC_BYTES = {"cfg4": 54275328}
+NCU_TRAFFIC_BYTES = {"cfg4": 54284800}
 # Small-network ensembles (cfg1, cfg2: one thread per trajectory, state in shared memory) are bound
 # by plain ALU issue, not memory.  Thread instructions per trajectory-step, from
 # `ncu --metrics smsp__thread_inst_executed.sum` over a whole launch:
