@@ -160,7 +160,7 @@ int rt_set_rate_schedule(rt_model *m, int32_t n_break, const double *t_break, co
  *   "ensemble_path"  0 = automatic, 1 = force one-thread-per-trajectory kernel,
  *                    2 = force the bundle (CTA-group-per-trajectory) kernel
  *   "state_mode"     0 = keep (T,P,a) in shared memory when a CTA's share fits (default),
- *                    1 = always stream it from global memory (the regime of M > ~1.1e6)
+ *                    1 = always stream it from global memory (the regime of M > ~1.3e6)
  *   "prefetch"       bit 0: L2 prefetch of the candidate's walk data, bit 1: speculative redraw,
  *                    bit 2: pre-walk of the exchange's runner-up (default 7 = all)
  *   "formulation"    0 = (T_k, P_k) internal-time form (default; the form every parity claim is

@@ -37,7 +37,7 @@ constexpr int kThreadKernelMaxM = 64; // one-thread-per-trajectory path: M, N at
 constexpr int kMinPairsPerCta = 256;  // do not spread a trajectory thinner than this
 constexpr int kBigDeg = 64;           // species read by more reactions than this get a block-offset table
 constexpr int kTargetBlocks = 256;    // ... with about this many reaction blocks
-constexpr size_t kSmemStateBytes = 208 * 1024;   // dynamic shared memory the (T,P,a) state may take
+constexpr size_t kSmemStateBytes = 210 * 1024;   // dynamic shared memory the (T,P,a) state may take
 
 #define CU_TRY(expr)                                                         \
   do {                                                                       \

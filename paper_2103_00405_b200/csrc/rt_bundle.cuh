@@ -5,7 +5,7 @@
 //
 // Every CTA owns a fixed contiguous range [k0, k1) of reactions.  Its (T, P, a) triples live
 //   * in SHARED MEMORY for the whole trajectory when the range fits (STATE_SMEM: M up to
-//     ~1.1e6 on 148 SMs) -- the per-firing pass then never leaves the SM;
+//     ~1.3e6 on 148 SMs) -- the per-firing pass then never leaves the SM;
 //   * in global memory otherwise (structure-of-arrays fp64, 16-byte vector accesses,
 //     24 B read + 8 B written per reaction per firing -- the HBM-streaming regime).
 //

@@ -500,3 +500,17 @@ def test_frozen_channels_boundary_condition(rt):
     frozen = mask.astype(bool)
     assert not g["fire_count"][frozen].any() and not g["T"][frozen].any()
     assert g["fire_count"][~frozen].sum() == 1500 and g["T"][~frozen].any()
+
+
+def test_shared_memory_capacity_edge(rt):
+    """The largest network whose state still fits in shared memory on 148 SMs (M = 1.3e6:
+    8 960 slots = 210 KB per CTA) and the first size that does not (M = 1.4e6 -> global memory)."""
+    for scale, smem in ((1.3, 1), (1.4, 0)):
+        net, x0, par = W.make_config("cfg4", scale=scale)
+        o = _oracle().run(net, x0, par["seed"], 0, 60, math.inf, 60)
+        with rt.Model(net) as m:
+            g = m.run(x0, par["seed"], 0, 60, math.inf, 60)
+            assert m.info("state_in_smem") == smem, (scale, m.info("state_in_smem"))
+        np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
+        np.testing.assert_array_equal(g["x"], o["x"])
+        np.testing.assert_allclose(g["trace_t"], o["trace_t"], rtol=RTOL_T, atol=0)
