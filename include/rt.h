@@ -107,6 +107,27 @@ int rt_run(rt_model *m, const int64_t *x0, uint64_t seed, uint64_t trajectory,
            uint64_t *fire_count_out, double *T_out, double *P_out,
            int32_t *trace_mu, double *trace_t, uint64_t trace_cap);
 
+/* Checkpoint / resume: continue a trajectory from the state an earlier rt_run (or rt_run_resume)
+ * returned -- x0 = its x_out, t0 = its res->t, T0 / P0 / fire_count0 [M] = its T_out / P_out /
+ * fire_count_out (all three required; in the residual formulation T0 = -R_k and P0 = 0, exactly as
+ * T_out / P_out deliver them).  Nothing is drawn at the start: the internal clocks T_k (Eq.15,
+ * PAPER.md:106) and the next internal firing times P_k (Eq.26) ARE the state of
+ * the random time-change representation, and later draws are keyed by (seed, trajectory, k,
+ * fire count), so rt_run to n1 firings followed by rt_run_resume for n2 - n1 more gives, bit for
+ * bit, what rt_run to n2 firings gives.  max_firings, the trace and res->firings count the
+ * firings of THIS call; res->t continues from t0; t_end is absolute.
+ * Errors as rt_run, plus RT_ERR_NULL (a state array missing), RT_ERR_BAD_ARG (t0 NaN, negative
+ * or beyond t_end; NaN in T0 / P0; a fire count >= 2^32) and RT_ERR_UNSUPPORTED (a rate schedule
+ * is set: whether a breakpoint at exactly t0 has acted is not part of the state).
+ * With "ensemble_path" = 1 a network small enough for it runs on the one-thread-per-trajectory
+ * kernel (no trace: RT_ERR_UNSUPPORTED if one is requested). */
+int rt_run_resume(rt_model *m, const int64_t *x0, double t0, const double *T0, const double *P0,
+                  const uint64_t *fire_count0, uint64_t seed, uint64_t trajectory,
+                  uint64_t max_firings, double t_end,
+                  int64_t *x_out, rt_result *res,
+                  uint64_t *fire_count_out, double *T_out, double *P_out,
+                  int32_t *trace_mu, double *trace_t, uint64_t trace_cap);
+
 /* Same trajectory, with x0 / x_out / trace_* DEVICE pointers on m's device and the work
  * enqueued on `stream` (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream; NULL = the
  * default stream).  res_dev: device pointer to one rt_result.  The call does not synchronise;
@@ -157,7 +178,9 @@ int rt_set_rate_schedule(rt_model *m, int32_t n_break, const double *t_break, co
  *   "refresh_mode"   0 = dependency-graph refresh of a_k (default), 1 = recompute every a_k
  *                    each firing (the paper's own GPU scheme)
  *   "bundle_ctas"    CTAs cooperating on one trajectory; 0 = choose automatically
- *   "ensemble_path"  0 = automatic, 1 = force one-thread-per-trajectory kernel,
+ *   "ensemble_path"  0 = automatic, 1 = force one-thread-per-trajectory kernel (RT_ERR_BAD_ARG at
+ *                    run time if the network is too large for it, RT_ERR_UNSUPPORTED together with
+ *                    a rate schedule or "formulation" = 1, which that kernel does not implement),
  *                    2 = force the bundle (CTA-group-per-trajectory) kernel
  *   "state_mode"     0 = keep (T,P,a) in shared memory when a CTA's share fits (default),
  *                    1 = always stream it from global memory (the regime of M > ~1.3e6)

@@ -27,6 +27,7 @@ def lib():
         _lib.oracle_binom.restype = C.c_int64
         _lib.oracle_binom.argtypes = [C.c_int64, C.c_int32]
         _lib.oracle_run.restype = C.c_int
+        _lib.oracle_run_from.restype = C.c_int
         _lib.oracle_run_residual.restype = C.c_int
         _lib.oracle_run_sched.restype = C.c_int
         _lib.oracle_ensemble.restype = C.c_int
@@ -106,6 +107,41 @@ def run(net, x0, seed, trajectory=0, max_firings=0, t_end=math.inf, trace_cap=0,
     nrec = min(int(firings.value), trace_cap)
     return dict(x=x, t=t.value, firings=int(firings.value), stop=int(stop.value), code=rc,
                 fire_count=fc, T=T, P=P,
+                trace_mu=None if tmu is None else tmu[:nrec],
+                trace_t=None if tt is None else tt[:nrec])
+
+
+def run_from(net, x0, t0, T0, P0, n0, seed, trajectory=0, max_firings=0, t_end=math.inf,
+             trace_cap=0, residual=False, check=True):
+    """One trajectory resumed from a checkpoint: real time t0, internal times T0, next internal
+    firing times P0, firings so far n0 (each array may be None = fresh).  residual=True: the
+    residual (Table 3) form; P0 then holds the residuals R_k and the result's "P" returns them."""
+    args, keep = _net_args(net)
+    N, M = int(net["n_species"]), int(net["n_reactions"])
+    x0 = np.ascontiguousarray(x0, dtype=np.int64)
+    T0 = None if T0 is None else np.ascontiguousarray(T0, dtype=np.float64)
+    P0 = None if P0 is None else np.ascontiguousarray(P0, dtype=np.float64)
+    n0 = None if n0 is None else np.ascontiguousarray(n0, dtype=np.uint64)
+    x = np.zeros(N, dtype=np.int64)
+    t = C.c_double(0.0)
+    firings = C.c_uint64(0)
+    stop = C.c_int32(0)
+    fc = np.zeros(M, dtype=np.uint64)
+    T = np.zeros(M, dtype=np.float64)
+    P = np.zeros(M, dtype=np.float64)
+    tmu = np.zeros(trace_cap, dtype=np.int32) if trace_cap else None
+    tt = np.zeros(trace_cap, dtype=np.float64) if trace_cap else None
+    rc = lib().oracle_run_from(*args, _p(x0, C.c_int64), C.c_double(t0), _p(T0, C.c_double),
+                               _p(P0, C.c_double), _p(n0, C.c_uint64), C.c_int32(1 if residual else 0),
+                               C.c_uint64(seed), C.c_uint64(trajectory), C.c_uint64(max_firings),
+                               C.c_double(t_end), _p(x, C.c_int64), C.byref(t), C.byref(firings),
+                               C.byref(stop), _p(fc, C.c_uint64), _p(T, C.c_double), _p(P, C.c_double),
+                               _p(tmu, C.c_int32), _p(tt, C.c_double), C.c_uint64(trace_cap))
+    if rc != 0 and check:
+        raise RuntimeError(f"oracle_run_from failed with code {rc}")
+    nrec = min(int(firings.value), trace_cap)
+    return dict(x=x, t=t.value, firings=int(firings.value), stop=int(stop.value), code=rc,
+                fire_count=fc, T=T, P=P, R=P if residual else None,
                 trace_mu=None if tmu is None else tmu[:nrec],
                 trace_t=None if tt is None else tt[:nrec])
 

@@ -27,12 +27,17 @@
 //                    (T_k, P_k) bookkeeping is reading G3 of DESIGN.md.
 //   nrrta_run_sched()     Eq.28 with piecewise-constant c_k(t)
 //   nrrta_run_residual()  Table 3 in residual-internal-time form (reading G4)
+//   Start / oracle_run_from()  the same two loops started from a checkpoint (t, T, P or R, n)
+//                    instead of step 0 -- no arithmetic of its own; pinned by the prefix identity
+//                    run(n1) + run_from(n2 - n1) == run(n2) and used to build exact finite ties
+//   apply_firing()   Eq.5 plus the count bound of reading G2 (Overflow)
 //   direct-method cross-check lives in tests/ (it must not share code with this file).
 //
 // Parity pins (tests/test_oracle_*.py): Philox known-answer vectors and the CUDA toolkit's
 // curand_Philox4x32_10; single-channel closed form t_n = sum E_i / c; birth-death
 // Poisson law; Kurtz identity Eq.5; invariants; race of exponentials; binomial factor;
-// brute-force Gillespie direct method on tiny networks.  Exact sample paths of the
+// brute-force Gillespie direct method on tiny networks; exact finite ties (reading G6) built from
+// rate_k = E(k,0) * 2^-3 and from checkpointed states.  Exact sample paths of the
 // large configs are fixed by no number in the paper: oracle<->GPU parity only.
 
 #include <cstdint>
@@ -111,6 +116,14 @@ double propensity(const Net &net, const int64_t *X, int32_t k) {
 enum { STOP_T_END = 1, STOP_MAX_FIRINGS = 2, STOP_ABSORBED = 3 };
 enum { OK = 0, ERR_BAD = -1, ERR_OVERFLOW = -5 };
 
+// Optional starting point of a run (checkpoint / resume): the state a previous run returned.
+// T, P (or R for the residual form) and n may each be NULL = fresh (T = 0, P = E(k, 0), n = 0).
+struct Start {
+  double t;
+  const double *T, *P;
+  const uint64_t *n;
+};
+
 int64_t count_bound(const Net &net) {
   int32_t smax = 1;
   for (int64_t e = 0; e < net.react_ptr[net.M]; ++e)
@@ -118,7 +131,21 @@ int64_t count_bound(const Net &net) {
   return smax <= 2 ? (((int64_t)1 << 31) - 1) : (((int64_t)1 << 21) - 1);
 }
 
-int nrrta_run(const Net &net, const int64_t *x0, uint64_t seed, uint64_t traj,
+// Step 6, X += v_mu (Eq.5), with the count bound of reading G2: if any count of the row would
+// leave [0, xmax] the whole update is skipped and the run ends with ERR_OVERFLOW (DESIGN.md
+// section 2, "Overflow": the firing is counted and traced, its internal-time increment and redraw
+// are applied, its change of X is not).
+int apply_firing(const Net &net, int64_t *X, int32_t mu, int64_t xmax) {
+  for (int64_t e = net.stoich_ptr[mu]; e < net.stoich_ptr[mu + 1]; ++e) {
+    const int64_t xj = X[net.stoich_species[e]] + net.stoich_v[e];
+    if (xj < 0 || xj > xmax) return ERR_OVERFLOW;
+  }
+  for (int64_t e = net.stoich_ptr[mu]; e < net.stoich_ptr[mu + 1]; ++e)
+    X[net.stoich_species[e]] += net.stoich_v[e];
+  return OK;
+}
+
+int nrrta_run(const Net &net, const int64_t *x0, const Start *start, uint64_t seed, uint64_t traj,
               uint64_t max_firings, double t_end,
               int64_t *x_out, double *t_out, uint64_t *firings_out, int32_t *stop_out,
               uint64_t *fire_count_out, double *T_out, double *P_out,
@@ -134,9 +161,16 @@ int nrrta_run(const Net &net, const int64_t *x0, uint64_t seed, uint64_t traj,
   std::vector<double> T(M, 0.0), P(M), a(M), dt(M);
   std::vector<uint32_t> n(M, 0u);
 
-  // step 0: T_k = 0, P_k = first internal firing time of the unit-rate process Y_k.
+  // step 0: T_k = 0, P_k = first internal firing time of the unit-rate process Y_k -- or the
+  // checkpointed values when the run resumes one.
   for (int32_t k = 0; k < M; ++k) P[k] = exp_draw(seed, traj, (uint32_t)k, 0u);
   double t = 0.0;
+  if (start) {
+    t = start->t;
+    if (start->T) for (int32_t k = 0; k < M; ++k) T[k] = start->T[k];
+    if (start->P) for (int32_t k = 0; k < M; ++k) P[k] = start->P[k];
+    if (start->n) for (int32_t k = 0; k < M; ++k) n[k] = (uint32_t)start->n[k];
+  }
   uint64_t fired = 0;
   int32_t stop = 0;
   int rc = OK;
@@ -172,12 +206,7 @@ int nrrta_run(const Net &net, const int64_t *x0, uint64_t seed, uint64_t traj,
     t = t + delta;
     for (int32_t k = 0; k < M; ++k) { const double inc = a[k] * delta; T[k] = T[k] + inc; }
     // step 6: X += v_mu (Eq.5).
-    for (int64_t e = net.stoich_ptr[mu]; e < net.stoich_ptr[mu + 1]; ++e) {
-      int64_t &xj = X[net.stoich_species[e]];
-      xj += net.stoich_v[e];
-      if (xj < 0) rc = ERR_BAD;            // cannot happen on a validated network
-      if (xj > xmax) rc = ERR_OVERFLOW;
-    }
+    rc = apply_firing(net, X.data(), mu, xmax);
     // step 7: only the fired channel gets a new internal-time target (Eq.26).
     n[mu] += 1u;
     P[mu] = P[mu] + exp_draw(seed, traj, (uint32_t)mu, n[mu]);
@@ -210,7 +239,7 @@ int nrrta_run(const Net &net, const int64_t *x0, uint64_t seed, uint64_t traj,
 //     Delta t_k = R_k / a_k,   R_k <- R_k - a_k * Delta t_mu for every k,   R_mu <- ln(1/r).
 // Same law as nrrta_run, different rounding (one array instead of two), so sample paths differ
 // in the last bits and eventually in the fired sequence: its own parity target.
-int nrrta_run_residual(const Net &net, const int64_t *x0, uint64_t seed, uint64_t traj,
+int nrrta_run_residual(const Net &net, const int64_t *x0, const Start *start, uint64_t seed, uint64_t traj,
                        uint64_t max_firings, double t_end,
                        int64_t *x_out, double *t_out, uint64_t *firings_out, int32_t *stop_out,
                        uint64_t *fire_count_out, double *R_out,
@@ -226,6 +255,11 @@ int nrrta_run_residual(const Net &net, const int64_t *x0, uint64_t seed, uint64_
   std::vector<uint32_t> n(M, 0u);
   for (int32_t k = 0; k < M; ++k) R[k] = exp_draw(seed, traj, (uint32_t)k, 0u);
   double t = 0.0;
+  if (start) {             // resume: start->P holds the checkpointed residuals R_k
+    t = start->t;
+    if (start->P) for (int32_t k = 0; k < M; ++k) R[k] = start->P[k];
+    if (start->n) for (int32_t k = 0; k < M; ++k) n[k] = (uint32_t)start->n[k];
+  }
   uint64_t fired = 0;
   int32_t stop = 0;
   int rc = OK;
@@ -254,12 +288,7 @@ int nrrta_run_residual(const Net &net, const int64_t *x0, uint64_t seed, uint64_
     }
     t = t + delta;
     for (int32_t k = 0; k < M; ++k) { const double dec = a[k] * delta; R[k] = R[k] - dec; }
-    for (int64_t e = net.stoich_ptr[mu]; e < net.stoich_ptr[mu + 1]; ++e) {
-      int64_t &xj = X[net.stoich_species[e]];
-      xj += net.stoich_v[e];
-      if (xj < 0) rc = ERR_BAD;
-      if (xj > xmax) rc = ERR_OVERFLOW;
-    }
+    rc = apply_firing(net, X.data(), mu, xmax);
     n[mu] += 1u;
     R[mu] = exp_draw(seed, traj, (uint32_t)mu, n[mu]);     // Table 3: a fresh ln(1/r) for mu only
     if (fired < trace_cap) {
@@ -360,12 +389,7 @@ int nrrta_run_sched(const Net &net, const int64_t *x0, uint64_t seed, uint64_t t
     }
     t = t + delta;
     for (int32_t k = 0; k < M; ++k) { const double inc = a[k] * delta; T[k] = T[k] + inc; }
-    for (int64_t e = net.stoich_ptr[mu]; e < net.stoich_ptr[mu + 1]; ++e) {
-      int64_t &xj = X[net.stoich_species[e]];
-      xj += net.stoich_v[e];
-      if (xj < 0) rc = ERR_BAD;
-      if (xj > xmax) rc = ERR_OVERFLOW;
-    }
+    rc = apply_firing(net, X.data(), mu, xmax);
     n[mu] += 1u;
     P[mu] = P[mu] + exp_draw(seed, traj, (uint32_t)mu, n[mu]);
     if (fired < trace_cap) {
@@ -415,7 +439,28 @@ int oracle_run(int32_t N, int32_t M, const int64_t *react_ptr, const int32_t *re
                int32_t *stop_out, uint64_t *fire_count_out, double *T_out, double *P_out,
                int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
   Net net{N, M, react_ptr, react_species, react_sigma, stoich_ptr, stoich_species, stoich_v, rate};
-  return nrrta_run(net, x0, seed, traj, max_firings, t_end, x_out, t_out, firings_out,
+  return nrrta_run(net, x0, nullptr, seed, traj, max_firings, t_end, x_out, t_out, firings_out,
+                   stop_out, fire_count_out, T_out, P_out, trace_mu, trace_t, trace_cap);
+}
+
+// Resume from a checkpoint (t0, T0, P0, n0 = fire counts so far; each array may be NULL = fresh).
+// residual != 0: the residual (Table 3) form, P0 = the residuals R_k, T0 unused, R returned in P_out.
+int oracle_run_from(int32_t N, int32_t M, const int64_t *react_ptr, const int32_t *react_species,
+                    const int32_t *react_sigma, const int64_t *stoich_ptr,
+                    const int32_t *stoich_species, const int32_t *stoich_v, const double *rate,
+                    const int64_t *x0, double t0, const double *T0, const double *P0,
+                    const uint64_t *n0, int32_t residual, uint64_t seed, uint64_t traj,
+                    uint64_t max_firings, double t_end, int64_t *x_out, double *t_out,
+                    uint64_t *firings_out, int32_t *stop_out, uint64_t *fire_count_out,
+                    double *T_out, double *P_out, int32_t *trace_mu, double *trace_t,
+                    uint64_t trace_cap) {
+  Net net{N, M, react_ptr, react_species, react_sigma, stoich_ptr, stoich_species, stoich_v, rate};
+  const Start st{t0, T0, P0, n0};
+  if (residual)
+    return nrrta_run_residual(net, x0, &st, seed, traj, max_firings, t_end, x_out, t_out,
+                              firings_out, stop_out, fire_count_out, P_out, trace_mu, trace_t,
+                              trace_cap);
+  return nrrta_run(net, x0, &st, seed, traj, max_firings, t_end, x_out, t_out, firings_out,
                    stop_out, fire_count_out, T_out, P_out, trace_mu, trace_t, trace_cap);
 }
 
@@ -441,7 +486,7 @@ int oracle_run_residual(int32_t N, int32_t M, const int64_t *react_ptr, const in
                         int32_t *stop_out, uint64_t *fire_count_out, double *R_out,
                         int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
   Net net{N, M, react_ptr, react_species, react_sigma, stoich_ptr, stoich_species, stoich_v, rate};
-  return nrrta_run_residual(net, x0, seed, traj, max_firings, t_end, x_out, t_out, firings_out,
+  return nrrta_run_residual(net, x0, nullptr, seed, traj, max_firings, t_end, x_out, t_out, firings_out,
                             stop_out, fire_count_out, R_out, trace_mu, trace_t, trace_cap);
 }
 
@@ -459,7 +504,7 @@ int oracle_ensemble(int32_t N, int32_t M, const int64_t *react_ptr, const int32_
   std::vector<int> codes(n_traj, 0);
   auto work = [&](uint64_t first, uint64_t step) {
     for (uint64_t i = first; i < n_traj; i += step)
-      codes[i] = nrrta_run(net, x0, seed, traj_first + i, max_firings, t_end,
+      codes[i] = nrrta_run(net, x0, nullptr, seed, traj_first + i, max_firings, t_end,
                            x_out + (size_t)i * (size_t)N, t_out + i, firings_out + i,
                            stop_out + i, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
   };

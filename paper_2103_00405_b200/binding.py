@@ -54,6 +54,7 @@ def lib():
     L.rt_validate_network.argtypes = [C.POINTER(_Network)]
     L.rt_create.argtypes = [C.POINTER(_Network), i32, C.POINTER(vp)]
     L.rt_run.argtypes = [vp, vp, u64, u64, u64, f64, vp, vp, vp, vp, vp, vp, vp, u64]
+    L.rt_run_resume.argtypes = [vp, vp, f64, vp, vp, vp, u64, u64, u64, f64, vp, vp, vp, vp, vp, vp, vp, u64]
     L.rt_run_dev.argtypes = [vp, vp, u64, u64, u64, f64, vp, vp, vp, vp, u64, vp]
     L.rt_ensemble.argtypes = [vp, vp, u64, u64, u64, u64, f64, vp, vp]
     L.rt_ensemble_dev.argtypes = [vp, vp, u64, u64, u64, u64, f64, vp, vp, vp]
@@ -65,7 +66,7 @@ def lib():
     L.rt_destroy.restype = None
     L.rt_strerror.argtypes = [i32]
     L.rt_strerror.restype = C.c_char_p
-    for name in ("rt_validate_network", "rt_create", "rt_run", "rt_run_dev", "rt_ensemble", "rt_set_rate_schedule",
+    for name in ("rt_validate_network", "rt_create", "rt_run", "rt_run_resume", "rt_run_dev", "rt_ensemble", "rt_set_rate_schedule",
                  "rt_ensemble_dev", "rt_sync", "rt_set_option", "rt_get_info"):
         getattr(L, name).restype = i32
     _lib = L
@@ -156,6 +157,32 @@ def rt_run(handle, x0, seed, trajectory, max_firings, t_end, n_species, n_reacti
     return rc, out
 
 
+def rt_run_resume(handle, x0, t0, T0, P0, fire_count0, seed, trajectory, max_firings, t_end,
+                  n_species, n_reactions, trace_cap=0, want_state=False):
+    """Host-pointer rt_run_resume.  Returns (code, dict) like rt_run."""
+    x0 = _np(x0, np.int64)
+    T0 = None if T0 is None else _np(T0, np.float64)
+    P0 = None if P0 is None else _np(P0, np.float64)
+    n0 = None if fire_count0 is None else _np(fire_count0, np.uint64)
+    x_out = np.zeros(n_species, dtype=np.int64)
+    res = np.zeros(1, dtype=RESULT_DTYPE)
+    fc = np.zeros(n_reactions, dtype=np.uint64) if want_state else None
+    T = np.zeros(n_reactions, dtype=np.float64) if want_state else None
+    P = np.zeros(n_reactions, dtype=np.float64) if want_state else None
+    tmu = np.zeros(trace_cap, dtype=np.int32) if trace_cap else None
+    tt = np.zeros(trace_cap, dtype=np.float64) if trace_cap else None
+    rc = lib().rt_run_resume(C.c_void_p(handle), _ptr(x0), float(t0), _ptr(T0), _ptr(P0), _ptr(n0),
+                             int(seed), int(trajectory), int(max_firings), float(t_end),
+                             _ptr(x_out), _ptr(res), _ptr(fc), _ptr(T), _ptr(P), _ptr(tmu), _ptr(tt),
+                             int(trace_cap))
+    nrec = min(int(res["firings"][0]), trace_cap)
+    out = dict(x=x_out, t=float(res["t"][0]), firings=int(res["firings"][0]),
+               stop=int(res["stop"][0]), status=int(res["status"][0]), fire_count=fc, T=T, P=P,
+               trace_mu=None if tmu is None else tmu[:nrec],
+               trace_t=None if tt is None else tt[:nrec])
+    return rc, out
+
+
 def rt_ensemble(handle, x0, seed, traj_first, n_traj, max_firings, t_end, n_species, want_x=True):
     """Host-pointer rt_ensemble.  Returns (code, dict(x[n_traj,N], t, firings, stop, status))."""
     x0 = _np(x0, np.int64)
@@ -238,6 +265,16 @@ class Model:
                          self.n_reactions, trace_cap, want_state)
         if check and rc != RT_OK:
             raise RtError(rc, "rt_run")
+        out["code"] = rc
+        return out
+
+    def run_resume(self, x0, t0, T0, P0, fire_count0, seed, trajectory=0, max_firings=0,
+                   t_end=math.inf, trace_cap=0, want_state=False, check=True):
+        rc, out = rt_run_resume(self.handle, x0, t0, T0, P0, fire_count0, seed, trajectory,
+                                max_firings, t_end, self.n_species, self.n_reactions, trace_cap,
+                                want_state)
+        if check and rc != RT_OK:
+            raise RtError(rc, "rt_run_resume")
         out["code"] = rc
         return out
 

@@ -83,7 +83,7 @@ struct rt_model {
   int sched_n = 0;
   bool sched_has_mask = false;
   // staging for the host-pointer API
-  DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t;
+  DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t, d_T0, d_P0, d_n0;
   // options
   int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0, opt_prefetch = 7, opt_formulation = 0;
   // info
@@ -150,6 +150,13 @@ int upload(DevBuf &buf, const std::vector<T> &host) {
   return RT_OK;
 }
 
+// Checkpoint a single trajectory resumes from (device pointers); all null = fresh start.
+struct StartDev {
+  double t0 = 0.0;
+  const double *T0 = nullptr, *P0 = nullptr;
+  const uint32_t *n0 = nullptr;
+};
+
 // How one launch is shaped: B bundles of S CTAs; smem = the (T,P,a) state lives in shared memory.
 struct Plan { int S, B, G; int pairs_per_cta; int cnt_pad; bool smem; };
 
@@ -205,7 +212,8 @@ int ensure_state(rt_model *m, const Plan &pl) {
 
 int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_first, u64 n_traj,
                    u64 max_firings, double t_end, long long *x_out_dev, rt_result *res_dev,
-                   int32_t *trace_mu_dev, double *trace_t_dev, u64 trace_cap, cudaStream_t st) {
+                   int32_t *trace_mu_dev, double *trace_t_dev, u64 trace_cap, cudaStream_t st,
+                   const StartDev &start = StartDev()) {
   const Plan pl = plan_bundles(m, n_traj);
   int rc = ensure_state(m, pl);
   if (rc != RT_OK) return rc;
@@ -218,13 +226,14 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.S = pl.S; p.B = pl.B; p.G = pl.G; p.pairs_per_cta = pl.pairs_per_cta; p.cnt_pad = pl.cnt_pad;
   p.x0 = x0_dev; p.seed = seed; p.traj_first = traj_first; p.n_traj = n_traj;
   p.max_firings = max_firings; p.t_end = t_end;
+  p.T0 = start.T0; p.P0 = start.P0; p.n0 = start.n0; p.t0 = start.t0;
   p.x_out = x_out_dev; p.res = res_dev;
   p.trace_mu = trace_mu_dev; p.trace_t = trace_t_dev;
   p.trace_cap = (trace_mu_dev || trace_t_dev) ? trace_cap : 0;
   p.refresh_mode = m->refresh_mode;
   p.prefetch = m->opt_prefetch;
   p.formulation = m->opt_formulation;
-  if (m->sched_n > 0 && (m->refresh_mode != 0 || m->opt_formulation != 0)) return RT_ERR_UNSUPPORTED;
+  if (m->sched_n > 0 && (m->refresh_mode != 0 || m->opt_formulation != 0 || start.T0)) return RT_ERR_UNSUPPORTED;
   p.sched_n = m->sched_n;
   p.sched_t = (const double *)m->d_sched_t.p;
   p.sched_f = (const double *)m->d_sched_f.p;
@@ -270,8 +279,11 @@ bool thread_path_fits(const rt_model *m) {
 
 int launch_threads(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_first, u64 n_traj,
                    u64 max_firings, double t_end, long long *x_out_dev, rt_result *res_dev,
-                   cudaStream_t st) {
+                   cudaStream_t st, const StartDev &start = StartDev(), double *T_out = nullptr,
+                   double *P_out = nullptr, uint32_t *n_out = nullptr) {
   rt::ThreadParams p{};
+  p.T0 = start.T0; p.P0 = start.P0; p.n0 = start.n0; p.t0 = start.t0;
+  p.T_out = T_out; p.P_out = P_out; p.n_out = n_out;
   p.net = m->net; p.nnz_r = m->nnz_r; p.nnz_v = m->nnz_v;
   p.x0 = x0_dev; p.seed = seed; p.traj_first = traj_first; p.n_traj = n_traj;
   p.max_firings = max_firings; p.t_end = t_end; p.x_out = x_out_dev; p.res = res_dev;
@@ -351,7 +363,8 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
     std::vector<uint32_t> cursor(dp.begin(), dp.end() - 1);
     for (int32_t k = 0; k < M; ++k) {
       const uint32_t rb = rp[k], re = rp[k + 1];
-      const int32_t j1 = rs[rb < re ? rb : 0], s1 = rg[rb < re ? rb : 0];
+      const bool has = rb < re;                  // (rs / rg are empty when no reaction has reactants)
+      const int32_t j1 = has ? rs[rb] : -1, s1 = has ? rg[rb] : 0;
       const int32_t j2 = (re - rb >= 2) ? rs[rb + 1] : -1, s2 = (re - rb >= 2) ? rg[rb + 1] : 0;
       const int32_t flags = s1 | (s2 << 8) | ((re - rb > 2) ? 0x10000 : 0);
       for (uint32_t e = rb; e < re; ++e) {
@@ -449,16 +462,23 @@ int rt_run_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t traje
                         (cudaStream_t)stream);
 }
 
-int rt_run(rt_model *m, const int64_t *x0, uint64_t seed, uint64_t trajectory,
-           uint64_t max_firings, double t_end, int64_t *x_out, rt_result *res,
-           uint64_t *fire_count_out, double *T_out, double *P_out,
-           int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
+// Body of rt_run / rt_run_resume (host pointers).  resume: start from (t0, T0, P0, n0).
+static int run_host(rt_model *m, const int64_t *x0, bool resume, double t0, const double *T0, const double *P0,
+             const uint64_t *n0, uint64_t seed, uint64_t trajectory, uint64_t max_firings, double t_end,
+             int64_t *x_out, rt_result *res, uint64_t *fire_count_out, double *T_out, double *P_out,
+             int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
   if (!m || !x0 || !res) return RT_ERR_NULL;
+  if (resume && (!T0 || !P0 || !n0)) return RT_ERR_NULL;
   int rc = check_limits(max_firings, t_end);
   if (rc != RT_OK) return rc;
   if ((rc = check_x0(m, x0)) != RT_OK) return rc;
-  CU_TRY(cudaSetDevice(m->device));
   const size_t N = (size_t)m->net.N, M = (size_t)m->net.M;
+  if (resume) {
+    if (!std::isfinite(t0) || t0 < 0.0 || t0 > t_end) return RT_ERR_BAD_ARG;
+    for (size_t k = 0; k < M; ++k)
+      if (std::isnan(T0[k]) || std::isnan(P0[k]) || n0[k] > 0xffffffffull) return RT_ERR_BAD_ARG;
+  }
+  CU_TRY(cudaSetDevice(m->device));
   if (!trace_mu && !trace_t) trace_cap = 0;
   if ((rc = m->d_x0.ensure(N * 8)) != RT_OK) return rc;
   if ((rc = m->d_xout.ensure(N * 8)) != RT_OK) return rc;
@@ -468,12 +488,38 @@ int rt_run(rt_model *m, const int64_t *x0, uint64_t seed, uint64_t trajectory,
     if ((rc = m->d_trace_t.ensure(trace_cap * 8)) != RT_OK) return rc;
   }
   cudaStream_t st = 0;
+  StartDev start;
+  if (resume) {
+    std::vector<uint32_t> n32(M);
+    for (size_t k = 0; k < M; ++k) n32[k] = (uint32_t)n0[k];
+    if ((rc = m->d_T0.ensure(M * 8)) != RT_OK) return rc;
+    if ((rc = m->d_P0.ensure(M * 8)) != RT_OK) return rc;
+    if ((rc = m->d_n0.ensure(M * 4)) != RT_OK) return rc;
+    CU_TRY(cudaMemcpy(m->d_T0.p, T0, M * 8, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(m->d_P0.p, P0, M * 8, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(m->d_n0.p, n32.data(), M * 4, cudaMemcpyHostToDevice));
+    start.t0 = t0;
+    start.T0 = (const double *)m->d_T0.p; start.P0 = (const double *)m->d_P0.p;
+    start.n0 = (const uint32_t *)m->d_n0.p;
+  }
   CU_TRY(cudaMemcpyAsync(m->d_x0.p, x0, N * 8, cudaMemcpyHostToDevice, st));
   CU_TRY(cudaMemsetAsync(m->d_res.p, 0, sizeof(rt_result), st));
-  rc = launch_bundles(m, (const long long *)m->d_x0.p, seed, trajectory, 1, max_firings, t_end,
-                      (long long *)m->d_xout.p, (rt_result *)m->d_res.p,
-                      trace_cap ? (int32_t *)m->d_trace_mu.p : nullptr,
-                      trace_cap ? (double *)m->d_trace_t.p : nullptr, trace_cap, st);
+  // "ensemble_path" = 1 sends a resumed single trajectory of a tiny network through the
+  // one-thread-per-trajectory kernel (which records no trace)
+  const bool threads = resume && m->opt_ensemble_path == 1;
+  if (threads) {
+    if (!thread_path_fits(m) || m->opt_formulation != 0 || m->sched_n > 0 || trace_cap) return RT_ERR_UNSUPPORTED;
+    const Plan pl = plan_bundles(m, 1);
+    if ((rc = ensure_state(m, pl)) != RT_OK) return rc;
+    rc = launch_threads(m, (const long long *)m->d_x0.p, seed, trajectory, 1, max_firings, t_end,
+                        (long long *)m->d_xout.p, (rt_result *)m->d_res.p, st, start,
+                        (double *)m->d_T.p, (double *)m->d_P.p, (uint32_t *)m->d_n.p);
+  } else {
+    rc = launch_bundles(m, (const long long *)m->d_x0.p, seed, trajectory, 1, max_firings, t_end,
+                        (long long *)m->d_xout.p, (rt_result *)m->d_res.p,
+                        trace_cap ? (int32_t *)m->d_trace_mu.p : nullptr,
+                        trace_cap ? (double *)m->d_trace_t.p : nullptr, trace_cap, st, start);
+  }
   if (rc != RT_OK) return rc;
   if ((rc = finish(m, st)) != RT_OK) return rc;
   CU_TRY(cudaMemcpy(res, m->d_res.p, sizeof(rt_result), cudaMemcpyDeviceToHost));
@@ -491,6 +537,23 @@ int rt_run(rt_model *m, const int64_t *x0, uint64_t seed, uint64_t trajectory,
   return res->status;
 }
 
+int rt_run(rt_model *m, const int64_t *x0, uint64_t seed, uint64_t trajectory,
+           uint64_t max_firings, double t_end, int64_t *x_out, rt_result *res,
+           uint64_t *fire_count_out, double *T_out, double *P_out,
+           int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
+  return run_host(m, x0, false, 0.0, nullptr, nullptr, nullptr, seed, trajectory, max_firings, t_end,
+                  x_out, res, fire_count_out, T_out, P_out, trace_mu, trace_t, trace_cap);
+}
+
+int rt_run_resume(rt_model *m, const int64_t *x0, double t0, const double *T0, const double *P0,
+                  const uint64_t *fire_count0, uint64_t seed, uint64_t trajectory,
+                  uint64_t max_firings, double t_end, int64_t *x_out, rt_result *res,
+                  uint64_t *fire_count_out, double *T_out, double *P_out,
+                  int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
+  return run_host(m, x0, true, t0, T0, P0, fire_count0, seed, trajectory, max_firings, t_end,
+                  x_out, res, fire_count_out, T_out, P_out, trace_mu, trace_t, trace_cap);
+}
+
 int rt_ensemble_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t traj_first,
                     uint64_t n_traj, uint64_t max_firings, double t_end, int64_t *x_out_dev,
                     rt_result *res_dev, void *stream) {
@@ -503,6 +566,8 @@ int rt_ensemble_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t 
   bool use_threads = thread_path_fits(m) && m->opt_formulation == 0 && m->sched_n == 0;
   if (m->opt_ensemble_path == 1) {
     if (!thread_path_fits(m)) return RT_ERR_BAD_ARG;
+    // the thread kernel implements the plain (T,P) form with constant rates only
+    if (m->opt_formulation != 0 || m->sched_n > 0) return RT_ERR_UNSUPPORTED;
     use_threads = true;
   } else if (m->opt_ensemble_path == 2) {
     use_threads = false;
@@ -621,16 +686,11 @@ void rt_destroy(rt_model *m) {
                     &m->d_sp_rec, &m->d_sp_big, &m->d_big_off, &m->d_dep,
                     &m->d_T, &m->d_P, &m->d_a, &m->d_n, &m->d_X, &m->d_exch, &m->d_err,
                     &m->d_x0, &m->d_xout, &m->d_res, &m->d_trace_mu, &m->d_trace_t,
+                    &m->d_T0, &m->d_P0, &m->d_n0,
                     &m->d_sched_t, &m->d_sched_f, &m->d_sched_mask};
   for (DevBuf *b : bufs) b->release();
   delete m;
 }
-
-#ifdef RT_PHASE_TIMING
-int rt_debug_dump(unsigned long long *out) {
-  return cudaMemcpyFromSymbol(out, rt::g_dbg, sizeof(unsigned long long) * 160 * 512 * 8) == cudaSuccess ? 0 : -1;
-}
-#endif
 
 const char *rt_strerror(int code) {
   switch (code) {

@@ -51,6 +51,10 @@ struct BundleParams {
   int cnt_pad;            // STATE_SMEM: slots per array (the CTA's reactions padded to a whole number
                           // of scan batches; padding slots hold a = T = 0, P = 1)
   const long long *x0;    // [N]
+  // checkpoint to resume from (rt_run_resume; single trajectory): nullptr = fresh start
+  const double *T0, *P0;  // [M]
+  const uint32_t *n0;     // [M]
+  double t0;              // real time of the checkpoint (0 for a fresh start)
   u64 seed, traj_first, n_traj, max_firings;
   double t_end;
   long long *x_out;       // [n_traj][N] or nullptr
@@ -69,28 +73,6 @@ struct BundleParams {
   const unsigned char *sched_mask;
   int *err;               // set to 1 on a barrier timeout
 };
-
-#ifdef RT_PHASE_TIMING
-#ifndef RT_PT_ALL
-#define RT_PT_ALL 0
-#endif
-constexpr bool getenv_all_ctas = RT_PT_ALL;
-__device__ unsigned long long g_dbg[160 * 512 * 8];   // [cta][firing][post, done, walk_done, stream_done] ns
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#if RT_PHASE_TIMING >= 2
-#define PT_DECL long long pt_acc[6] = {0, 0, 0, 0, 0, 0}; long long pt_last = clock64();
-#define PT_G(slot) { if (gen < 512 && lane == 0) g_dbg[((size_t)r * 512 + gen) * 8 + (slot)] = gtime(); }
-#define PT_MARK(i) { long long now_ = clock64(); pt_acc[i] += now_ - pt_last; pt_last = now_; }
-#else
-#define PT_DECL long long pt_acc[6] = {0, 0, 0, 0, 0, 0};
-#define PT_G(slot)
-#define PT_MARK(i)
-#endif
-#else
-#define PT_DECL
-#define PT_G(slot)
-#define PT_MARK(i)
-#endif
 
 constexpr long long kSpinLimitCycles = 6000000000ll;   // ~3 s: a barrier that long is a bug
 
@@ -493,9 +475,6 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
       const uint32_t tag = gen + 1u;
       const u64 par = (u64)(((gen >> 1) & 1u) ^ 1u) << 63;     // never matches zeroed memory
       u64 *buf = exch + (size_t)(gen & 1u) * (size_t)p.S * kSlotStride;
-#ifdef RT_PHASE_TIMING
-      if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 0] = gtime();
-#endif
       if (lane == 0)
         st_relaxed_v2(buf + (size_t)kSlotStride * r, (u64)__double_as_longlong(c.dt) | par,
                       ((u64)tag << 32) | (u64)(uint32_t)c.k);
@@ -524,9 +503,6 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
         if (pending && clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); c.k = -2; break; }
       }
       const bool timed_out = __any_sync(0xffffffffu, c.k == -2);
-#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING >= 2
-      if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 1] = gtime();
-#endif
       const Cand mine_best = c;
       c = warp_lexmin(c);
       // runner-up = best of everything but the winner: the likeliest winner of the next firing
@@ -650,7 +626,6 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   __shared__ Cand redo[SMEM ? 1 : BLOCK];            // global-memory state: cooperative re-scan results
   __shared__ short stale_list[SMEM ? 1 : BLOCK];
   extern __shared__ __align__(16) unsigned char dyn_smem[];
-  PT_DECL
   const NetDev &net = p.net;
   const int tid = threadIdx.x, lane = tid & 31;
   const bool is_walker = tid >= NT;
@@ -700,19 +675,25 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     gen += 1u;
     for (int k = k0 + tid; k < (SMEM ? k0 + cnt_pad : k1); k += BLOCK) {
       double a0 = 0.0, p0 = 1.0;     // padding: a = 0, P - T = 1 > 0, so its q~ is +inf, never NaN
+      double t_init = 0.0, p_init = 1.0;
+      uint32_t n_init = 0u;
       if (k < k1 && k < M) {
         a0 = propensity(net, X, k);
-        p0 = exp_draw(p.seed, traj, (uint32_t)k, 0u);
         if (filter_unsafe(a0)) ctx.any_odd = 1;
-      }
-      const double t_init = resid ? -p0 : 0.0, p_init = resid ? 0.0 : p0;   // residual form: T = -R
+        if (p.T0) {                                   // resume: the checkpointed internal times
+          t_init = __ldg(p.T0 + k); p_init = __ldg(p.P0 + k); n_init = __ldg(p.n0 + k);
+        } else {
+          p0 = exp_draw(p.seed, traj, (uint32_t)k, 0u);
+          t_init = resid ? -p0 : 0.0; p_init = resid ? 0.0 : p0;            // residual form: T = -R
+        }
+      } else if (resid) { t_init = -1.0; p_init = 0.0; }
       if (SMEM) { sT[k - k0] = t_init; sP[k - k0] = p_init; sA[k - k0] = a0; }
       else { __stcg(T + k, t_init); __stcg(P + k, p_init); __stcg(A + k, a0); }
-      if (k < k1) nfire[k] = 0u;
+      if (k < k1) nfire[k] = n_init;
     }
     __syncthreads();
 
-    double t = 0.0, dprev = 0.0;
+    double t = p.t0, dprev = 0.0;
     u64 fired = 0;
     int mu_prev = -1, stop = 0, status = RT_OK;
     bool finishing = false;
@@ -722,10 +703,6 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     constexpr bool full = FULL;
 
     for (;;) {   // one iteration per firing, plus one closing pass
-      PT_MARK(5)
-#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING >= 2
-      if (tid == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 7] = gtime();
-#endif
       // walker-warp state of this firing (uniform over the warp)
       Ranges rg;
 #pragma unroll
@@ -755,10 +732,6 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(net.srow) + (size_t)mu_prev * 4 + lane);
         }
         w_csr = __shfl_sync(0xffffffffu, ent.x, 0) == -2;
-#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING == 1
-        if (lane == 0 && gen < 512) g_dbg[((size_t)r * 512 + gen) * 8 + 3] = hit ? 1ull : 0ull;
-#endif
-        PT_G(4)
         if (hit) {
           // One L2 round trip: the X words of the changed species and of the reactants of the
           // first 32 pre-walked entries are loaded together; a word that does not yet carry this
@@ -815,7 +788,6 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           }
           if (active) xn = x_peek(X, ent.x, ent.y, fired, net.xmax, done);
           const bool bad = __any_sync(0xffffffffu, active && xn < 0);
-          PT_G(5)
           if (bad) { if (lane == 0) ctx.abort_local = 1; }
           else if (active && !done) atomicMax(X + ent.x, x_pack(fired, xn));
           uint32_t acc = 0;
@@ -866,11 +838,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           }
         }
         __syncwarp();                            // this warp's X updates precede its reads below
-        PT_G(6)
       }
       if (full && mu_prev >= 0) __syncthreads(); // full recompute reads the new X in the stream
 
-      PT_MARK(0)
       bool first_round = true;
       for (;;) {   // rounds: one, unless this CTA has more than kListCap refreshes
         if (is_walker) {
@@ -908,17 +878,10 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           mybest_k[tid] = defer ? -3 : best.k;
           if (defer) dirty[tid] = 1;
         }
-        PT_MARK(1)
-#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING >= 2
-        if (gen < 512 && first_round && (tid == 0 || tid == NT)) g_dbg[((size_t)r * 512 + gen) * 8 + (tid == NT ? 2 : 3)] = gtime();
-#endif
         __syncthreads();
         // ----- apply the staged refreshes; mark the owning threads for a re-scan
         const int n = ctx.list_n;
         const bool more = ctx.more != 0;
-#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING == 1
-        if (tid == 0 && gen < 512 && first_round) g_dbg[((size_t)r * 512 + gen) * 8 + 2] = (unsigned long long)n;
-#endif
         // A refreshed reaction invalidates its owner's proposal only if it IS that proposal (the
         // proposal is the minimum over the owner's other, unchanged reactions as well).  Then the
         // owner re-scans; otherwise the new waiting time simply joins the reduction as one more
@@ -950,7 +913,6 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         if (!more) break;
         first_round = false;
       }
-      PT_MARK(2)
       if (SCHED && rate_change) {
         // the pass above brought every T_k to the breakpoint with the old rates; now switch
         rate_change = false;
@@ -1025,9 +987,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       if (finishing) break;
 
       // ---- a-3 argmin over the bundle
-      PT_MARK(3)
       const Cand win = bundle_argmin<BLOCK, SMEM>(p, ctx, exch, nfire, r, gen, best, spec);
-      PT_MARK(4)
       if (win.k == -2) return;
 
       // ---- a-4 stop tests, identical in every thread of every CTA of the bundle
@@ -1066,13 +1026,6 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       }
     }
 
-#if defined(RT_PHASE_TIMING) && RT_PHASE_TIMING >= 2
-    if ((tid == 0 || tid == NT) && (getenv_all_ctas || r == 0 || r == p.S - 1 || r == p.S / 2))
-      printf("cta %d %s: updates %.0f  %s %.0f  barrier+apply %.0f  rescan %.0f  argmin+exchange %.0f  stop tests %.0f cyc/firing\n",
-             r, tid == 0 ? "stream thread" : "walker", (double)pt_acc[0] / fired,
-             tid == 0 ? "stream" : "walk", (double)pt_acc[1] / fired, (double)pt_acc[2] / fired,
-             (double)pt_acc[3] / fired, (double)pt_acc[4] / fired, (double)pt_acc[5] / fired);
-#endif
     // ---- trajectory done: every CTA's X updates are visible bundle-wide after the fenced barrier
     if (!bundle_barrier<BLOCK>(exch, p.S, r, gen, p.err)) return;
     gen += 1u;

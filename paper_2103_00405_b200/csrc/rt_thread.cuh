@@ -20,6 +20,13 @@ struct ThreadParams {
   double t_end;
   long long *x_out;      // [n_traj][N] or nullptr
   rt_result *res;        // [n_traj]
+  // single trajectory through this kernel (rt_run_resume with ensemble_path = 1): checkpoint to
+  // start from and final per-reaction state; all nullptr for ensembles
+  const double *T0, *P0;
+  const uint32_t *n0;
+  double t0;
+  double *T_out, *P_out;
+  uint32_t *n_out;
 };
 
 // Shared-memory bytes: network copy + BLOCK * (3*8*M + 4*M + 8*N).
@@ -66,11 +73,11 @@ __global__ void __launch_bounds__(BLOCK) rt_thread_kernel(const ThreadParams p) 
 #define ST(arr, i) arr[(size_t)(i) * BLOCK + tid]
   for (int j = 0; j < N; ++j) ST(sX, j) = p.x0[j];
   for (int k = 0; k < M; ++k) {
-    ST(sT, k) = 0.0;
-    ST(sP, k) = exp_draw(p.seed, traj, (uint32_t)k, 0u);
-    ST(sN, k) = 0u;
+    ST(sT, k) = p.T0 ? p.T0[k] : 0.0;
+    ST(sP, k) = p.T0 ? p.P0[k] : exp_draw(p.seed, traj, (uint32_t)k, 0u);
+    ST(sN, k) = p.T0 ? p.n0[k] : 0u;
   }
-  double t = 0.0;
+  double t = p.t0;
   u64 fired = 0;
   int stop = 0, status = RT_OK;
 
@@ -98,12 +105,13 @@ __global__ void __launch_bounds__(BLOCK) rt_thread_kernel(const ThreadParams p) 
     // a-5
     t = __dadd_rn(t, delta);
     for (int k = 0; k < M; ++k) ST(sT, k) = __dadd_rn(ST(sT, k), __dmul_rn(ST(sA, k), delta));
-    // a-6
+    // a-6: nothing is written if any count of the row would leave [0, xmax] (as in the bundle kernel)
     for (uint32_t e = s_sp[mu]; e < s_sp[mu + 1]; ++e) {
       const long long x = ST(sX, s_ss[e]) + (long long)s_sv[e];
       if (x < 0 || x > net.xmax) status = RT_ERR_OVERFLOW;
-      ST(sX, s_ss[e]) = x;
     }
+    if (status == RT_OK)
+      for (uint32_t e = s_sp[mu]; e < s_sp[mu + 1]; ++e) ST(sX, s_ss[e]) += (long long)s_sv[e];
     // a-7
     const uint32_t c = ST(sN, mu) + 1u;
     ST(sN, mu) = c;
@@ -115,6 +123,8 @@ __global__ void __launch_bounds__(BLOCK) rt_thread_kernel(const ThreadParams p) 
 
   if (p.x_out)
     for (int j = 0; j < N; ++j) p.x_out[it * (u64)N + (u64)j] = ST(sX, j);
+  if (p.T_out && it == 0)
+    for (int k = 0; k < M; ++k) { p.T_out[k] = ST(sT, k); p.P_out[k] = ST(sP, k); p.n_out[k] = ST(sN, k); }
   rt_result res;
   res.t = t; res.firings = fired; res.stop = stop; res.status = status;
   p.res[it] = res;

@@ -2,11 +2,13 @@
 same seeded inputs.  Bar (BASELINE.json north_star): fired-reaction sequence and species counts
 bit-exact for the first 1e4 firings, event times within 1e-12 relative."""
 import math
+import os
 
 import numpy as np
 import pytest
 
 import rt_workloads as W
+from helpers.tie_cases import tie_network, expected_trace
 
 pytestmark = pytest.mark.gpu
 
@@ -132,16 +134,157 @@ def test_extreme_rates_and_cubic_reactions(rt, ctas):
 
 def test_count_overflow_is_reported(rt):
     """0 -> X from the count bound: after the three deaths of the other species the first birth
-    leaves [0, 2^31-1] -> RT_ERR_OVERFLOW at firing 4."""
+    leaves [0, 2^31-1] -> RT_ERR_OVERFLOW at firing 4.  DESIGN.md 2 "Overflow": the offending
+    firing is counted and traced, its X change is not applied -- on the bundle kernel, on the
+    one-thread-per-trajectory kernel and in the oracle alike."""
     net = W.from_reactions(2, [({}, {0: 1}, 1.0), ({1: 1}, {}, 1.0)])
     x0 = np.array([2**31 - 1, 3], dtype=np.int64)
     o = _oracle().run(net, x0, 5, 0, 100, math.inf, 100, check=False)
     with rt.Model(net) as m:
-        g = m.run(x0, 5, 0, 100, math.inf, 100, check=False)
+        g = m.run(x0, 5, 0, 100, math.inf, 100, want_state=True, check=False)
+        ens = []
+        for path in (1, 2):
+            m.set_option("ensemble_path", path)
+            ens.append(m.ensemble(x0, 5, 0, 3, 100, math.inf, check=False))
+            assert m.info("ensemble_path") == path
     assert g["code"] == rt.RT_ERR_OVERFLOW and g["status"] == rt.RT_ERR_OVERFLOW
     assert o["code"] == -5 and g["firings"] == o["firings"] == 4
     np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
-    np.testing.assert_array_equal(g["x"], [2**31 - 1, 0])   # the offending update is not applied
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["x"], [2**31 - 1, 0])
+    np.testing.assert_array_equal(g["fire_count"], o["fire_count"])
+    for e in ens:                      # row i of an ensemble == rt_run(trajectory i), errors included
+        assert e["code"] == rt.RT_ERR_OVERFLOW and (e["status"] == rt.RT_ERR_OVERFLOW).all()
+        for i in range(3):
+            oi = _oracle().run(net, x0, 5, i, 100, math.inf, 0, check=False)
+            np.testing.assert_array_equal(e["x"][i], oi["x"])
+            assert e["firings"][i] == oi["firings"]
+
+
+def test_network_without_any_reactant(rt):
+    """A validated network with NO reactant entries at all (pure sources: empty react_species /
+    react_sigma arrays): the single-channel closed form t_n = sum_i E_i / c (Eq.23-24,
+    PAPER.md:156-160) through the bundle kernel and through the thread kernel."""
+    c, n = 2.5, 200
+    net = W.from_reactions(1, [({}, {0: 1}, c)])
+    assert net["react_species"].size == 0
+    g, o = _check_run(rt, net, np.array([0]), 13, 6, n, math.inf, n)
+    e = [_oracle().exp_draw(13, 6, 0, i) for i in range(n)]
+    np.testing.assert_allclose(g["trace_t"], np.cumsum(e) / c, rtol=1e-12)
+    net3 = W.from_reactions(3, [({}, {0: 1}, 1.0), ({}, {1: 1, 2: 1}, 0.3), ({}, {2: 2}, 2.0)])
+    _check_run(rt, net3, np.zeros(3, dtype=np.int64), 2, 0, 500, math.inf, 500)
+    o = _oracle().ensemble(net3, np.zeros(3, dtype=np.int64), 2, 0, 40, 300, math.inf)
+    with rt.Model(net3) as m:
+        e = m.ensemble(np.zeros(3, dtype=np.int64), 2, 0, 40, 300, math.inf)
+        assert m.info("ensemble_path") == 1
+    np.testing.assert_array_equal(e["x"], o["x"])
+    np.testing.assert_allclose(e["t"], o["t"], rtol=RTOL_T)
+
+
+# ------------------------------------------------------------------ exact ties (reading G6)
+def _check_tie(rt, M, coupled, formulation, options, n_more=40):
+    """Exact finite ties from a checkpointed state (tests/helpers/tie_cases.py): an M-way tie at
+    dt = 8, then M-1 firings that tie at dt = 0.  The expected trace 0, 1, ..., M-1 at t = 8.0
+    follows by hand; the oracle is compared as well, past the end of the tie."""
+    net, x0, T0, P0, n0 = tie_network(M, coupled=coupled)
+    n = M + n_more
+    o = _oracle().run_from(net, x0, 0.0, T0, P0, n0, 9, 1, n, math.inf, n, residual=bool(formulation))
+    with rt.Model(net) as m:
+        m.set_option("formulation", formulation)
+        for name, val in options:
+            m.set_option(name, val)
+        if formulation:
+            g = m.run_resume(x0, 0.0, -P0, np.zeros(M), n0, 9, 1, n, math.inf, n, want_state=True)
+        else:
+            g = m.run_resume(x0, 0.0, T0, P0, n0, 9, 1, n, math.inf, n, want_state=True)
+    mu, tt = expected_trace(M)
+    np.testing.assert_array_equal(g["trace_mu"][:M], mu)
+    np.testing.assert_array_equal(g["trace_t"][:M], tt)
+    np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["fire_count"], o["fire_count"])
+    np.testing.assert_allclose(g["trace_t"], o["trace_t"], rtol=RTOL_T, atol=0)
+
+
+@pytest.mark.parametrize("formulation", [0, 1])
+@pytest.mark.parametrize("state_mode", [0, 1])
+@pytest.mark.parametrize("ctas", [1, 3, 7, 0])
+def test_exact_ties_go_to_the_lowest_index(rt, ctas, state_mode, formulation):
+    """north_star: "argmin reduction over k with ties broken by lowest index".  The ties straddle
+    the reactions of one thread (filter fallback: every approximate quotient of a thread is equal),
+    lanes, warps and CTAs (REDUX lexmin, exchange slots), and with `coupled` every firing refreshes
+    every hub reader inside the tie (fresh-candidate merge, warp-shared / cooperative re-scan)."""
+    opts = [("bundle_ctas", ctas), ("state_mode", state_mode)]
+    _check_tie(rt, 5003, False, formulation, opts)
+    _check_tie(rt, 4999, True, formulation, opts)
+
+
+def test_exact_ties_full_recompute_and_thread_kernel(rt):
+    _check_tie(rt, 1201, True, 0, [("refresh_mode", 1)])
+    # one-thread-per-trajectory kernel: no trace there, so the order shows in the counts --
+    # after j firings exactly the channels 0..j-1 have fired once, all at t = 8.0
+    M = 40
+    net, x0, T0, P0, n0 = tie_network(M, coupled=True)
+    with rt.Model(net) as m:
+        m.set_option("ensemble_path", 1)
+        for j in (1, 2, 17, M):
+            g = m.run_resume(x0, 0.0, T0, P0, n0, 9, 1, j, math.inf, want_state=True)
+            assert m.info("ensemble_path") == 1
+            assert g["t"] == 8.0 and g["firings"] == j
+            np.testing.assert_array_equal(g["fire_count"], (np.arange(M) < j).astype(np.uint64))
+            o = _oracle().run_from(net, x0, 0.0, T0, P0, n0, 9, 1, j, math.inf)
+            np.testing.assert_array_equal(g["x"], o["x"])
+            np.testing.assert_allclose(g["P"], o["P"], rtol=1e-12)
+
+
+@pytest.mark.parametrize("formulation,state_mode", [(0, 0), (0, 1), (1, 0), (1, 1)])
+def test_resume_continues_bit_for_bit(rt, formulation, state_mode):
+    """rt_run to n1 firings + rt_run_resume for n2 - n1 more == rt_run to n2 (include/rt.h), and
+    both equal the oracle; also across a t_end stop."""
+    net, x0, par = W.make_config("cfg3", scale=0.02)
+    with rt.Model(net) as m:
+        m.set_option("formulation", formulation)
+        m.set_option("state_mode", state_mode)
+        a = m.run(x0, 7, 4, 700, math.inf, 700, want_state=True)
+        b = m.run_resume(a["x"], a["t"], a["T"], a["P"], a["fire_count"], 7, 4, 800, math.inf, 800,
+                         want_state=True)
+        c = m.run(x0, 7, 4, 1500, math.inf, 1500, want_state=True)
+        t_end = float(c["trace_t"][1100]) * 1.0000001
+        d = m.run_resume(a["x"], a["t"], a["T"], a["P"], a["fire_count"], 7, 4, 0, t_end, 4096)
+    np.testing.assert_array_equal(b["trace_mu"], c["trace_mu"][700:])
+    np.testing.assert_array_equal(b["trace_t"], c["trace_t"][700:])
+    for key in ("x", "fire_count", "T", "P"):
+        np.testing.assert_array_equal(b[key], c[key])
+    assert b["t"] == c["t"] and b["firings"] == 800
+    assert d["stop"] == rt.RT_STOP_T_END and d["t"] == t_end and d["firings"] == 401
+    run = _oracle().run_residual if formulation else _oracle().run
+    o = run(net, x0, 7, 4, 1500, math.inf, 1500)
+    np.testing.assert_array_equal(c["trace_mu"], o["trace_mu"])
+
+
+def test_resume_argument_checks(rt):
+    net, x0 = W.lotka_volterra()
+    z = np.zeros(3)
+    n0 = np.zeros(3, dtype=np.uint64)
+    with rt.Model(net) as m:
+        assert m.run_resume(x0, 0.0, None, z, n0, 1, 0, 10, check=False)["code"] == rt.RT_ERR_NULL
+        assert m.run_resume(x0, -1.0, z, z, n0, 1, 0, 10, check=False)["code"] == rt.RT_ERR_BAD_ARG
+        assert m.run_resume(x0, 5.0, z, z, n0, 1, 0, 10, 2.0, check=False)["code"] == rt.RT_ERR_BAD_ARG
+        bad = z.copy(); bad[1] = math.nan
+        assert m.run_resume(x0, 0.0, bad, z, n0, 1, 0, 10, check=False)["code"] == rt.RT_ERR_BAD_ARG
+        big = n0.copy(); big[2] = 2**32
+        assert m.run_resume(x0, 0.0, z, z, big, 1, 0, 10, check=False)["code"] == rt.RT_ERR_BAD_ARG
+        m.set_rate_schedule([0.5], [2.0])
+        assert m.run_resume(x0, 0.0, z, z + 1, n0, 1, 0, 10, check=False)["code"] == rt.RT_ERR_UNSUPPORTED
+        # the thread kernel implements neither schedules nor the residual form: forcing it must
+        # fail loudly instead of returning constant-rate (T, P) results
+        m.set_option("ensemble_path", 1)
+        assert m.ensemble(x0, 2, 0, 4, 100, check=False)["code"] == rt.RT_ERR_UNSUPPORTED
+        m.set_rate_schedule([], [])
+        m.set_option("formulation", 1)
+        assert m.ensemble(x0, 2, 0, 4, 100, check=False)["code"] == rt.RT_ERR_UNSUPPORTED
+        m.set_option("formulation", 0)
+        assert m.ensemble(x0, 2, 0, 4, 100)["code"] == rt.RT_OK
 
 
 def test_cfg3_full_first_1e4(rt):
@@ -164,32 +307,57 @@ def test_cfg4_full_first_1e4(rt):
     assert g["firings"] == 10_000
 
 
-def test_cfg5a_full_size_prefix(rt):
-    """BASELINE config 5a (M=1e7: state streamed from global memory) at full size; the oracle
-    does 20 firings (2e8 reaction-steps) in seconds."""
+def test_cfg5a_full_size_full_length(rt):
+    """BASELINE config 5a (N=1e6, M=1e7: state streamed from global memory, 512-thread CTAs,
+    cooperative re-scan) at full size and full length: all 2 000 firings, in both formulations,
+    everything _check_run compares.  (The oracle needs ~2 min per formulation; the two run side
+    by side on two host threads.)"""
+    from concurrent.futures import ThreadPoolExecutor
     net, x0, par = W.make_config("cfg5a")
-    with rt.Model(net) as m:
-        g = m.run(x0, par["seed"], 0, 20, math.inf, 20, want_state=True)
-        assert m.info("state_in_smem") == 0
-    o = _oracle().run(net, x0, par["seed"], 0, 20, math.inf, 20)
-    np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
-    np.testing.assert_array_equal(g["x"], o["x"])
-    np.testing.assert_allclose(g["trace_t"], o["trace_t"], rtol=RTOL_T, atol=0)
+    n = par["max_firings"]
+    assert n == 2000 and net["n_reactions"] == 10_000_000
+    with ThreadPoolExecutor(2) as ex:
+        fo = ex.submit(_oracle().run, net, x0, par["seed"], 0, n, math.inf, n)
+        fr = ex.submit(_oracle().run_residual, net, x0, par["seed"], 0, n, math.inf, n)
+        with rt.Model(net) as m:
+            g = m.run(x0, par["seed"], 0, n, math.inf, n, want_state=True)
+            assert m.info("state_in_smem") == 0 and m.info("bundle_ctas") == m.info("num_sms")
+            m.set_option("formulation", 1)
+            gr = m.run(x0, par["seed"], 0, n, math.inf, n, want_state=True)
+        o, orr = fo.result(), fr.result()
+    for a, b in ((g, o), (gr, orr)):
+        assert a["firings"] == b["firings"] == n and a["stop"] == b["stop"]
+        np.testing.assert_array_equal(a["trace_mu"], b["trace_mu"])
+        np.testing.assert_array_equal(a["x"], b["x"])
+        np.testing.assert_array_equal(a["fire_count"], b["fire_count"])
+        np.testing.assert_allclose(a["trace_t"], b["trace_t"], rtol=RTOL_T, atol=0)
+        assert math.isclose(a["t"], b["t"], rel_tol=RTOL_T, abs_tol=0)
     np.testing.assert_allclose(g["T"], o["T"], rtol=1e-10, atol=1e-12)
+    np.testing.assert_allclose(g["P"], o["P"], rtol=1e-12, atol=0)
+    np.testing.assert_allclose(-gr["T"], orr["R"], rtol=1e-10, atol=1e-12)
 
 
-def test_cfg5b_full_size_ensemble_prefix(rt):
+def test_cfg5b_full_size_ensemble(rt):
     """BASELINE config 5b: 64 trajectories of the M=1e5 network in the bench launch shape
-    (several bundles with on-chip state); every row against the oracle for 250 firings."""
+    (several bundles with on-chip state); every row against the oracle for 2 500 firings, and
+    trajectory 0 traced through rt_run in the same bundle shape."""
     net, x0, par = W.make_config("cfg5b")
-    n = 64
-    o = _oracle().ensemble(net, x0, par["seed"], 0, n, 250, math.inf, n_threads=8)
+    n, firings = 64, 2500
+    o = _oracle().ensemble(net, x0, par["seed"], 0, n, firings, math.inf, n_threads=os.cpu_count() or 8)
+    o0 = _oracle().run(net, x0, par["seed"], 0, firings, math.inf, firings)
     with rt.Model(net) as m:
-        g = m.ensemble(x0, par["seed"], 0, n, 250, math.inf)
+        g = m.ensemble(x0, par["seed"], 0, n, firings, math.inf)
         assert m.info("ensemble_path") == 2 and m.info("state_in_smem") == 1
+        shape = m.info("bundle_ctas")
+        m.set_option("bundle_ctas", shape)
+        g0 = m.run(x0, par["seed"], 0, firings, math.inf, firings)
     np.testing.assert_array_equal(g["x"], o["x"])
     np.testing.assert_array_equal(g["firings"], o["firings"])
+    np.testing.assert_array_equal(g["stop"], o["stop"])
     np.testing.assert_allclose(g["t"], o["t"], rtol=RTOL_T)
+    np.testing.assert_array_equal(g0["trace_mu"], o0["trace_mu"])
+    np.testing.assert_allclose(g0["trace_t"], o0["trace_t"], rtol=RTOL_T, atol=0)
+    np.testing.assert_array_equal(g0["x"], g["x"][0])
 
 
 def test_t_end_stop_and_absorption(rt):
@@ -263,10 +431,20 @@ def test_prefix_property(rt):
 
 # ------------------------------------------------------------------ beyond the bit-exact horizon
 def _ks_and_moments(a, b):
+    """Two-sample KS p-value, and the differences of the means and of the variances in units of
+    their standard errors (north_star: "means and variances within 3 standard errors").  The
+    sampling variance of s^2 is (m4 - s^4 (n-3)/(n-1)) / n for any law with a fourth moment."""
     from scipy import stats
     p = stats.ks_2samp(a, b).pvalue
     se = math.sqrt(a.var(ddof=1) / len(a) + b.var(ddof=1) / len(b))
-    return p, abs(a.mean() - b.mean()) / max(se, 1e-300)
+
+    def var_of_var(x):
+        n, s2 = len(x), x.var(ddof=1)
+        m4 = ((x - x.mean()) ** 4).mean()
+        return max(m4 - s2 * s2 * (n - 3) / (n - 1), 0.0) / n
+    se_v = math.sqrt(var_of_var(a) + var_of_var(b))
+    return (p, abs(a.mean() - b.mean()) / max(se, 1e-300),
+            abs(a.var(ddof=1) - b.var(ddof=1)) / max(se_v, 1e-300))
 
 
 def test_cfg1_ensemble_statistics(rt):
@@ -287,8 +465,8 @@ def test_cfg1_ensemble_statistics(rt):
     xg, xo = other["x"][:, 0].astype(float), o["x"][:, 0].astype(float)
     assert abs(xg.mean() - 100.0) < 3 * math.sqrt(100.0 / n)
     assert abs(xg.var(ddof=1) - 100.0) < 3 * 100.0 * math.sqrt(2.0 / (n - 1)) + 3 * math.sqrt(100.0 / n)
-    p, z = _ks_and_moments(xg, xo)
-    assert p > 0.01 and z < 3.0
+    p, z, zv = _ks_and_moments(xg, xo)
+    assert p > 0.01 and z < 3.0 and zv < 3.0
     # exact law: KS against the Poisson(100) CDF is conservative for a discrete law
     assert stats.kstest(xg, stats.poisson(100).cdf).pvalue > 0.01
 
@@ -296,7 +474,9 @@ def test_cfg1_ensemble_statistics(rt):
 def test_cfg2_ensemble_statistics(rt):
     """BASELINE config 2 shape (Lotka-Volterra, one thread per trajectory), t_end = 1 (~3e4 firings
     per trajectory): same seed -> identical rows; different seed -> both species' marginals agree
-    with the oracle's (means within 3 SE, KS p > 0.01, Holm over the two species)."""
+    with the oracle's (means and variances within 3 SE, KS p > 0.01, Holm over the two species).
+    The config's own size (1e5 trajectories to t_end = 10, 3e10 steps) is bench.py's cfg2 run, far
+    beyond what the oracle can follow; this is the same path at a size it can."""
     net, x0, par = W.make_config("cfg2")
     n = 400
     o = _oracle().ensemble(net, x0, par["seed"], 0, n, par["max_firings"], 1.0, n_threads=8)
@@ -308,13 +488,13 @@ def test_cfg2_ensemble_statistics(rt):
     np.testing.assert_array_equal(same["firings"], o["firings"])
     ps = []
     for j in range(2):
-        p, z = _ks_and_moments(other["x"][:, j].astype(float), o["x"][:, j].astype(float))
-        assert z < 3.0
+        p, z, zv = _ks_and_moments(other["x"][:, j].astype(float), o["x"][:, j].astype(float))
+        assert z < 3.0 and zv < 3.0, (j, z, zv)
         ps.append(p)
     ps.sort()
     assert ps[0] > 0.01 / 2 and ps[1] > 0.01      # Holm-corrected
-    fz = _ks_and_moments(other["firings"].astype(float), o["firings"].astype(float))[1]
-    assert fz < 3.0
+    _, fz, fzv = _ks_and_moments(other["firings"].astype(float), o["firings"].astype(float))
+    assert fz < 3.0 and fzv < 3.0
 
 
 # ------------------------------------------------------------------ residual (Table 3) formulation
@@ -478,11 +658,11 @@ def test_cfg3_scaled_ensemble_beyond_the_bit_exact_horizon(rt):
     np.testing.assert_allclose(same["t"], o["t"], rtol=1e-11)
     ps = []
     for j in species:
-        p, z = _ks_and_moments(other["x"][:, j].astype(float), o["x"][:, j].astype(float))
-        assert z < 3.5, (j, z)
+        p, z, zv = _ks_and_moments(other["x"][:, j].astype(float), o["x"][:, j].astype(float))
+        assert z < 3.0 and zv < 3.0, (j, z, zv)
         ps.append(p)
-    p, z = _ks_and_moments(other["t"], o["t"])
-    assert z < 3.5
+    p, z, zv = _ks_and_moments(other["t"], o["t"])
+    assert z < 3.0 and zv < 3.0, (z, zv)
     ps.append(p)
     for rank, p in enumerate(sorted(ps)):
         assert p > 0.01 / (len(ps) - rank), (rank, p)      # Holm step-down

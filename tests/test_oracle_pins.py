@@ -19,6 +19,7 @@ import oracle
 import rt_workloads as W
 from helpers.direct_method import direct_method
 from helpers.exact_kurtz import exact_path
+from helpers.tie_cases import tie_network, expected_trace
 from helpers.rta_table1 import rta_table1
 
 HERE = os.path.dirname(os.path.abspath(__file__))
@@ -187,11 +188,87 @@ def test_matches_exact_rational_path(case):
 
 
 def test_tie_goes_to_lowest_index():
-    """Reading G6: equal waiting times -> lowest k.  Two channels whose clamped residual is 0
-    (reading G7) tie at Delta t = 0; +inf ties (all a_k = 0) mean ABSORBED."""
+    """Reading G6 (Eq.25 says nothing about ties): equal waiting times -> the
+    lowest k fires.  Source reactions 0 -> X_k with c_k = E(seed, traj, k, 0) * 2^-3: a_k = c_k and
+    P_k = E_k, so dt_k = E_k / (E_k * 2^-3) = 8.0 EXACTLY for every k (a finite M-way tie); after
+    channel 0 fires, T_k = c_k * 8 = E_k exactly, so every other residual is exactly 0 (reading G7)
+    and the next M-1 firings are ties at dt = 0.  Expected by hand: mu = 0, 1, ..., M-1, all at
+    t = 8.0.  A `<=` instead of `<` in step 3 gives M-1, M-2, ... and fails here (mutation-checked
+    when this test was written)."""
+    seed, traj = 3, 2
+    for M in (2, 6, 37):
+        rate = [oracle.exp_draw(seed, traj, k, 0) * 2.0 ** -3 for k in range(M)]
+        net = W.from_reactions(M, [({}, {k: 1}, rate[k]) for k in range(M)])
+        x0 = [0] * M
+        runs = [oracle.run(net, x0, seed, traj, M + 5, math.inf, M + 5),
+                oracle.run_residual(net, x0, seed, traj, M + 5, math.inf, M + 5),
+                oracle.run_sched(net, x0, seed, traj, M + 5, math.inf, M + 5,
+                                 t_break=[100.0], factor=[2.0])]
+        for r in runs:
+            assert list(r["trace_mu"][:M]) == list(range(M))
+            assert list(r["trace_t"][:M]) == [8.0] * M
+            assert r["trace_t"][M] > 8.0                 # the tie is over: fresh draws
+    # +inf ties (every a_k = 0) mean ABSORBED, not a firing of channel 0
     net = W.from_reactions(1, [({0: 1}, {}, 1.0), ({0: 1}, {}, 2.0)])
     r = oracle.run(net, [0], seed=1, max_firings=5)
     assert (r["firings"], r["stop"]) == (0, oracle.STOP_ABSORBED)
+
+
+@pytest.mark.parametrize("coupled", [False, True])
+@pytest.mark.parametrize("residual", [False, True])
+def test_tie_from_checkpointed_state(coupled, residual):
+    """The same exact ties built from a checkpoint (tests/helpers/tie_cases.py: P_k = 8 a_k(X0),
+    T_k = 0) instead of from the draws -- the form the GPU parity test uses, because it does not
+    depend on the last bit of a logarithm.  With `coupled` every firing changes the hub species,
+    so every reader's propensity changes inside the tie: 0 / a_new is still 0."""
+    M = 41
+    net, x0, T0, P0, n0 = tie_network(M, coupled=coupled)
+    r = oracle.run_from(net, x0, 0.0, T0, P0, n0, 9, 1, M + 20, math.inf, M + 20, residual=residual)
+    mu, tt = expected_trace(M)
+    assert list(r["trace_mu"][:M]) == list(mu) and list(r["trace_t"][:M]) == list(tt)
+    assert r["trace_t"][M] > 8.0 and r["firings"] == M + 20
+    assert (r["fire_count"] >= 1).all()
+
+
+@pytest.mark.parametrize("residual", [False, True])
+def test_resume_is_a_prefix_identity(residual):
+    """run to n1, then run_from the returned state for n2 - n1 more == run to n2, bit for bit:
+    (X, t, T, P, n) is the whole state of the random time-change representation (Eq.15-16,
+    PAPER.md:106-110), and later draws are keyed by the fire counts (Eq.26)."""
+    net, x0, par = W.make_config("cfg3", scale=0.01)
+    run = oracle.run_residual if residual else oracle.run
+    a = run(net, x0, 7, 4, 400, math.inf, 400)
+    c = run(net, x0, 7, 4, 1000, math.inf, 1000)
+    if residual:
+        b = oracle.run_from(net, a["x"], a["t"], None, a["R"], a["fire_count"], 7, 4, 600, math.inf, 600,
+                            residual=True)
+        assert np.array_equal(b["R"], c["R"])
+    else:
+        b = oracle.run_from(net, a["x"], a["t"], a["T"], a["P"], a["fire_count"], 7, 4, 600, math.inf, 600)
+        assert np.array_equal(b["T"], c["T"]) and np.array_equal(b["P"], c["P"])
+    assert np.array_equal(b["trace_mu"], c["trace_mu"][400:])
+    assert np.array_equal(b["trace_t"], c["trace_t"][400:])
+    assert np.array_equal(b["x"], c["x"]) and np.array_equal(b["fire_count"], c["fire_count"])
+    assert b["t"] == c["t"]
+    # a time limit is absolute: resuming with the same t_end stops where the single run stops
+    t_end = float(c["trace_t"][700]) * 1.0000001
+    d = run(net, x0, 7, 4, 0, t_end)
+    if not residual:
+        e = oracle.run_from(net, a["x"], a["t"], a["T"], a["P"], a["fire_count"], 7, 4, 0, t_end)
+        assert e["t"] == d["t"] == t_end and e["firings"] + 400 == d["firings"] == 701
+        assert np.array_equal(e["T"], d["T"])
+
+
+def test_count_bound_stops_the_run_without_applying_the_update():
+    """Reading G2 bounds the counts (2^31 - 1 when every sigma <= 2); DESIGN.md 2 "Overflow": the
+    firing that would leave the bound is counted and traced, its X change is not applied."""
+    net = W.from_reactions(2, [({}, {0: 1}, 1.0), ({1: 1}, {}, 1.0)])
+    r = oracle.run(net, [2**31 - 1, 3], 5, 0, 100, math.inf, 100, check=False)
+    assert r["code"] == -5
+    assert r["trace_mu"][-1] == 0 and r["firings"] == len(r["trace_mu"])
+    deaths = int((r["trace_mu"] == 1).sum())
+    assert list(r["x"]) == [2**31 - 1, 3 - deaths]
+    assert r["fire_count"][0] == 1
 
 
 # ------------------------------------------------------------------ P3/P4: birth-death
