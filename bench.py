@@ -34,11 +34,15 @@ BYTES_PER_REACTION_FIRING = 32   # read T, P, a; write T (DESIGN.md "algorithmic
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the bundle kernel, from the
 # `ncu --set full` capture of this command (profiles/r1_v7_bundle_kernel.md): 51.56 MB + 2.73 MB.
 # Far BELOW the algorithmic bytes: at M = 1e6 the (T,P,a) state lives in shared memory.
-NCU_TRAFFIC_BYTES = {"cfg4": 54284800}
+NCU_TRAFFIC = {"cfg4": {"bytes": 54284800, "source": "profiles/r1_v7_bundle_kernel.md (ncu --set full, one launch)"}}
 # Small-network ensembles (cfg1, cfg2: one thread per trajectory, state in shared memory) are bound
 # by plain ALU issue, not memory.  Thread instructions per trajectory-step, from
 # `ncu --metrics smsp__thread_inst_executed.sum` over a whole launch:
 THREAD_INSTR_PER_STEP = {"cfg1": 382.0, "cfg2": 511.2}
+THREAD_INSTR_SOURCE = "profiles/r1_thread_kernel.md (ncu smsp__thread_inst_executed.sum / steps of one launch)"
+# the other BASELINE.json configs, reported in the same JSON line under "secondary"
+SECONDARY = ["cfg5a", "cfg5b", "cfg3", "cfg2"]
+SECONDARY_STEPS = 2
 # issue peak: 148 SMs x 4 schedulers x 32 lanes x 1.965 GHz (B200_PROFILING.md unit counts / clocks)
 ALU_PEAK_GINSTR = 148 * 4 * 32 * 1.965
 
@@ -53,6 +57,8 @@ def parse_args():
     ap.add_argument("--firings", type=int, default=0, help="firings per step (0 = the config's)")
     ap.add_argument("--scale", type=float, default=1.0, help="shrink N, M (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", dest="secondary", action="store_false",
+                    help="skip the secondary workloads (cfg5a, cfg5b, cfg3, cfg2)")
     ap.add_argument("--option", action="append", default=[], help="name=value for rt_set_option")
     ap.add_argument("--breakpoints", type=int, default=0,
                     help="time-dependent rates (Eq.28): this many rate breakpoints spread over the step")
@@ -148,47 +154,53 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def run_cuda(args):
-    import torch
-    import torch.distributed as dist
-    import paper_2103_00405_b200 as rt
+def smem_roofline(M, kernel_s_per_firing, sm_mhz, num_sms, bytes_per_reaction):
+    """The binding on-chip resource when (T, P, a) live in shared memory: aggregate shared-memory
+    bandwidth = SMs x 128 B/clk x SM clock (B200_PROFILING.md unit counts)."""
+    peak = num_sms * 128.0 * sm_mhz * 1e6 / 1e9                    # GB/s
+    ach = bytes_per_reaction * M / kernel_s_per_firing / 1e9
+    return {"smem_achieved": ach, "smem_peak": peak, "smem_frac": ach / peak,
+            "smem_peak_source": f"{num_sms} SMs x 128 B/clk x {sm_mhz:.0f} MHz"}
 
-    rt.lib()                                   # no extension -> ImportError; there is no fallback
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+def measure(rt, torch, dist, args, workload, steps, warmup, rank, world, local, headline):
+    """K device-timed steps of one workload (CUDA events on the launching stream, L2 flushed
+    between steps, clocks sampled during the timed region).  Returns the fields of a bench line."""
     dev = torch.device("cuda", local)
-
-    net, x0, par = W.make_config(args.workload, scale=args.scale)
+    scale = args.scale
+    net, x0, par = W.make_config(workload, scale=scale)
     N, M = int(net["n_species"]), int(net["n_reactions"])
-    firings = args.firings or par["max_firings"]
-    n_traj = par["n_traj"]
-    t_end = float(par.get("t_end", math.inf)) if args.workload in ("cfg1", "cfg2") else math.inf
+    firings = (args.firings if headline else 0) or par["max_firings"]
+    n_all = par["n_traj"]
+    t_end = float(par.get("t_end", math.inf)) if workload in ("cfg1", "cfg2") else math.inf
     seed = par["seed"]
-    traj0 = rank * n_traj                       # replicas: every rank its own trajectory ids
+    if n_all > 1 and world > 1:
+        # ensembles shard by trajectory id with no data-path collective (DESIGN.md 8): strong scaling
+        first, n_traj = rt.shard_range(n_all, rank, world)
+        traj0, scaling = first, "strong"
+    else:
+        n_traj, traj0, scaling = n_all, rank * n_all, "weak"      # replicas: own trajectory ids
     model = rt.Model(net, local)
     formulation = 0
-    for kv in args.option:
-        k, v = kv.split("=")
-        model.set_option(k, int(v))
-        if k == "formulation":
-            formulation = int(v)
+    if headline:
+        for kv in args.option:
+            k, v = kv.split("=")
+            model.set_option(k, int(v))
+            if k == "formulation":
+                formulation = int(v)
 
     x0_dev = torch.from_numpy(x0).to(dev)
-    x_out_dev = torch.empty(n_traj * N, dtype=torch.int64, device=dev)
-    res_dev = torch.zeros(n_traj * 3, dtype=torch.int64, device=dev)          # rt_result[n_traj]
-    trace_cap = min(firings, par.get("trace", 0)) if n_traj == 1 else 0
+    x_out_dev = torch.empty(max(n_traj, 1) * N, dtype=torch.int64, device=dev)
+    res_dev = torch.zeros(max(n_traj, 1) * 3, dtype=torch.int64, device=dev)   # rt_result[n_traj]
+    trace_cap = min(firings, par.get("trace", 0)) if n_all == 1 else 0
     tmu_dev = torch.empty(max(trace_cap, 1), dtype=torch.int32, device=dev)
     tt_dev = torch.empty(max(trace_cap, 1), dtype=torch.float64, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)              # > 126 MB L2
 
     def step_dev():
-        if n_traj == 1:
+        if n_traj == 0:
+            return
+        if n_all == 1:
             rc = rt.rt_run_dev(model.handle, x0_dev, seed, traj0, firings, t_end, x_out_dev,
                                res_dev, tmu_dev, tt_dev, trace_cap)
         else:
@@ -202,35 +214,39 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    if args.breakpoints > 0:
+    breakpoints = args.breakpoints if headline else 0
+    if breakpoints > 0:
         # learn how long (in simulated time) a step is, then spread the breakpoints over it:
         # factors alternate 1.5 / 0.5 on the even-numbered reactions
         step_dev()
         torch.cuda.synchronize()
         t_final = float(res_dev.cpu().numpy().view(rt.RESULT_DTYPE)["t"].max())
-        nb = args.breakpoints
-        tb = [t_final * (i + 1) / (nb + 2) for i in range(nb)]
-        fa = [1.5 if i % 2 == 0 else 0.5 for i in range(nb)]
+        tb = [t_final * (i + 1) / (breakpoints + 2) for i in range(breakpoints)]
+        fa = [1.5 if i % 2 == 0 else 0.5 for i in range(breakpoints)]
         model.set_rate_schedule(tb, fa, (np.arange(M) % 2 == 0).astype(np.uint8))
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(warmup, 3)):
         flush.fill_(1)
         step_dev()
     torch.cuda.synchronize()
     if rt.rt_sync(model.handle) != rt.RT_OK:
         raise SystemExit("bench.py: device reported an error during warm-up")
-    done = res_dev.cpu().numpy().view(rt.RESULT_DTYPE)
+    done = res_dev.cpu().numpy().view(rt.RESULT_DTYPE)[:n_traj]
     assert (done["status"] == 0).all(), done
     if math.isinf(t_end):
         assert (done["firings"] == firings).all(), done
-    else:
+    elif n_traj:
         # (a Lotka-Volterra trajectory may also die out -> absorbed, or explode -> max_firings)
         assert (done["stop"] >= rt.RT_STOP_T_END).all() and (done["stop"] == rt.RT_STOP_T_END).mean() > 0.9, done
-    fired_per_step = int(done["firings"].sum())      # trajectory-steps of one step (all trajectories)
+    fired_local = int(done["firings"].sum())         # trajectory-steps of one step on this rank
+    fired_t = torch.tensor([fired_local], dtype=torch.int64, device=dev)
+    if world > 1:
+        dist.all_reduce(fired_t)
+    fired_per_step = int(fired_t.item())             # ... on all ranks
 
     # ---- timed region: K steps, device-timed; per-step events bracket the kernel launch only
     # (L2 flush sits between steps, outside the per-step events but inside the barrier bracket).
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-          for _ in range(args.steps)]
+          for _ in range(steps)]
     launches0 = model.info("kernel_launches")
     sampler = ClockSampler(local) if rank == 0 else None
     barrier()
@@ -247,101 +263,157 @@ def run_cuda(args):
     if world > 1:
         dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
     total_s = float(total_ms.item()) * 1e-3
-    units = fired_per_step * args.steps * world
-    value = units / total_s
+    value = fired_per_step * steps / total_s
 
-    # ---- e2e: the host-pointer C-ABI call a user makes; copies inside the timed region
-    x0_pin = torch.from_numpy(x0.copy()).pin_memory().numpy()
-    e2e_tr = trace_cap
+    out = {"workload": workload, "value": value, "ms_per_step": 1e3 * total_s / steps,
+           "scaling": scaling, "gpu_launches": int(launches), "clocks": clocks}
+    if headline:
+        # ---- e2e: the host-pointer C-ABI call a user makes; copies inside the timed region
+        x0_pin = torch.from_numpy(x0.copy()).pin_memory().numpy()
 
-    def step_host():
-        if n_traj == 1:
-            out = model.run(x0_pin, seed, traj0, firings, t_end, trace_cap=e2e_tr)
-            return out["firings"]
-        out = model.ensemble(x0_pin, seed, traj0, n_traj, firings, t_end)
-        return int(out["firings"].sum())
+        def step_host():
+            if n_traj == 0:
+                return 0
+            if n_all == 1:
+                return model.run(x0_pin, seed, traj0, firings, t_end, trace_cap=trace_cap)["firings"]
+            return int(model.ensemble(x0_pin, seed, traj0, n_traj, firings, t_end)["firings"].sum())
 
-    step_host()
-    barrier()
-    t0 = time.perf_counter()
-    got = 0
-    for _ in range(args.steps):
-        got += step_host()
-    torch.cuda.synchronize()
-    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
-    e2e_value = got * world / float(e2e_s.item())
-    h2d = N * 8
-    d2h = n_traj * N * 8 + n_traj * 24 + e2e_tr * 12
+        step_host()
+        barrier()
+        t0 = time.perf_counter()
+        got = 0
+        for _ in range(steps):
+            got += step_host()
+        torch.cuda.synchronize()
+        e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        got_t = torch.tensor([got], dtype=torch.int64, device=dev)
+        if world > 1:
+            dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+            dist.all_reduce(got_t)
+        out["e2e"] = {"value": int(got_t.item()) / float(e2e_s.item()), "unit": UNIT,
+                      "h2d_bytes_per_step": N * 8,
+                      "d2h_bytes_per_step": n_traj * N * 8 + n_traj * 24 + trace_cap * 12}
 
     if rank == 0:
         peak, peak_src = peaks()
-        kernel_s = (sum(step_ms) / len(step_ms)) * 1e-3          # one bundle-kernel launch per step
-        # residual (Table 3) form: T and a read, T written -- no P: 24 bytes per reaction
-        alg_bytes = (24 if formulation else BYTES_PER_REACTION_FIRING) * M * fired_per_step
-        achieved = alg_bytes / kernel_s / 1e9
-        line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * total_s / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic",
-            "config": {"workload": args.workload, "n_species": N, "n_reactions": M,
-                       "trajectories_per_step": n_traj, "firings_per_step": fired_per_step,
-                       "parallelism": "replicas only (one trajectory per GPU)" if n_traj == 1
-                       else "independent trajectories", "l2": "flushed between steps (256 MB fill)",
-                       "bundle_ctas": model.info("bundle_ctas"), "bundles": model.info("bundles"),
-                       "block_threads": model.info("block_threads"),
-                       "state_in_shared_memory": bool(model.info("state_in_smem")),
-                       "us_per_firing": 1e6 * kernel_s / fired_per_step * n_traj,
-                       "ensemble_path": model.info("ensemble_path"),
-                       "formulation": "residual (Table 3)" if formulation else "(T, P) internal time",
-                       "rate_breakpoints": args.breakpoints},
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": d2h},
-            "gpu_launches": int(launches),
-            "clocks": clocks,
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
-                         "kernel": "rt_bundle_kernel", "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": alg_bytes,
-                         "frac_of_8TBs_nominal": achieved / 8000.0,
-                         "note": ("state (T,P,a) resident in shared memory: `achieved` is algorithmic "
-                                  "bytes per second, not DRAM throughput (see `traffic`); the step is "
-                                  "latency-bound (DESIGN.md 7)") if model.info("state_in_smem")
-                         else "state streamed from global memory: DRAM traffic = algorithmic bytes"},
-        }
-        if args.workload in THREAD_INSTR_PER_STEP:
+        kernel_s = (sum(step_ms) / len(step_ms)) * 1e-3          # one kernel launch per step (this rank)
+        smem = bool(model.info("state_in_smem"))
+        bundles = max(1, model.info("bundles"))
+        us_per_firing = 1e6 * kernel_s / max(fired_local, 1) * max(n_traj, 1)
+        out["config"] = {
+            "workload": workload, "n_species": N, "n_reactions": M,
+            "trajectories_per_step": n_all, "firings_per_step": fired_per_step,
+            "parallelism": ("replicas only (one trajectory per GPU)" if n_all == 1 else
+                            "independent trajectories" + (", sharded by trajectory id" if world > 1 else "")),
+            "l2": "flushed between steps (256 MB fill)",
+            "bundle_ctas": model.info("bundle_ctas"), "bundles": model.info("bundles"),
+            "block_threads": model.info("block_threads"), "state_in_shared_memory": smem,
+            "us_per_firing": us_per_firing, "ensemble_path": model.info("ensemble_path"),
+            "formulation": "residual (Table 3)" if formulation else "(T, P) internal time",
+            "rate_breakpoints": breakpoints}
+        if workload in THREAD_INSTR_PER_STEP:
             # one thread per trajectory, state in shared memory: plain ALU issue is the bound
-            ginstr = THREAD_INSTR_PER_STEP[args.workload] * fired_per_step / kernel_s / 1e9
-            line["roofline"] = {"bound": "alu", "achieved": ginstr, "peak": ALU_PEAK_GINSTR,
-                                "unit": "Ginstr/s", "frac": ginstr / ALU_PEAK_GINSTR, "traffic": None,
-                                "kernel": "rt_thread_kernel",
-                                "peak_source": "148 SMs x 4 schedulers x 32 lanes x 1.965 GHz (DESIGN.md 7)",
-                                "thread_instructions_per_step": THREAD_INSTR_PER_STEP[args.workload]}
-        if not args.no_cpu_baseline and world == 1:
-            if n_traj == 1:
-                sample = max(20, min(firings, int(1e9 // M)))    # ~1e9 reaction-steps: 10-30 s
-                v, dt = oracle_leg(net, x0, seed, traj0, sample)
-                line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                        "sample": f"first {sample} firings of {args.workload} "
-                                                  f"(M={M}), {dt:.1f} s, single thread"}
+            ginstr = THREAD_INSTR_PER_STEP[workload] * fired_local / kernel_s / 1e9
+            out["roofline"] = {"bound": "alu", "achieved": ginstr, "peak": ALU_PEAK_GINSTR,
+                               "unit": "Ginstr/s", "frac": ginstr / ALU_PEAK_GINSTR, "traffic": None,
+                               "kernel": "rt_thread_kernel",
+                               "peak_source": "148 SMs x 4 schedulers x 32 lanes x 1.965 GHz (DESIGN.md 7)",
+                               "thread_instructions_per_step": THREAD_INSTR_PER_STEP[workload],
+                               "thread_instructions_source": THREAD_INSTR_SOURCE}
+        else:
+            # residual (Table 3) form: T and a read, T written -- no P: 24 bytes per reaction
+            bpr = 24 if formulation else BYTES_PER_REACTION_FIRING
+            alg_bytes = bpr * M * fired_local
+            achieved = alg_bytes / kernel_s / 1e9
+            tr = NCU_TRAFFIC.get(workload)
+            roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": tr["bytes"] if tr else None,
+                    "traffic_source": tr["source"] if tr else None,
+                    "kernel": "rt_bundle_kernel", "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": alg_bytes,
+                    "frac_of_8TBs_nominal": achieved / 8000.0}
+            if smem:
+                sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+                # all bundles stream side by side: per-firing time of the chip = kernel_s / firings of
+                # one bundle's queue; aggregate bytes per second is what the shared memories deliver
+                roof.update(smem_roofline(M, kernel_s / max(fired_local, 1), sm_mhz,
+                                          model.info("num_sms"), bpr))
+                roof["note"] = ("state (T,P,a) resident in shared memory: `achieved` is algorithmic bytes "
+                                "per second, not DRAM throughput (see `traffic`); the binding resource is "
+                                "shared-memory bandwidth + the per-firing latency chain: `smem_frac` "
+                                "(DESIGN.md 7)")
             else:
-                # ensembles: one independent oracle instance per host core on a subset of the
-                # trajectories, sized for ~1e9 reaction-steps in total
-                import oracle
-                cores = os.cpu_count() or 1
-                per_traj = max(1, fired_per_step // n_traj) * M
-                sub = int(max(cores, min(n_traj, 1e9 // per_traj)))
-                t0 = time.perf_counter()
-                o = oracle.ensemble(net, x0, seed, traj0, sub, firings, t_end, n_threads=cores)
-                dt = time.perf_counter() - t0
-                line["cpu_baseline"] = {"value": float(o["firings"].sum()) / dt, "unit": UNIT,
-                                        "cores": cores, "kind": "oracle",
-                                        "sample": f"trajectories {traj0}..{traj0 + sub - 1} of {args.workload} "
-                                                  f"in full, {dt:.1f} s, one oracle instance per core"}
-        print(json.dumps(line))
+                roof["note"] = "state streamed from global memory: DRAM traffic = algorithmic bytes"
+            out["roofline"] = roof
+        out["_cpu"] = (net, x0, seed, traj0, firings, t_end, n_traj, fired_local, M)
     model.close()
+    del flush, x0_dev, x_out_dev, res_dev
+    torch.cuda.empty_cache()
+    return out
+
+
+def cpu_baseline(workload, net, x0, seed, traj0, firings, t_end, n_traj, fired_local, M):
+    """The oracle as it stands on the box's host cores, on a bounded sample (~1e9 reaction-steps)."""
+    if n_traj == 1:
+        sample = max(20, min(firings, int(1e9 // M)))    # ~1e9 reaction-steps: 10-30 s
+        v, dt = oracle_leg(net, x0, seed, traj0, sample)
+        return {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                "sample": f"first {sample} firings of {workload} (M={M}), {dt:.1f} s, single thread"}
+    # ensembles: one independent oracle instance per host core on a subset of the trajectories,
+    # sized for ~1e9 reaction-steps in total
+    import oracle
+    cores = os.cpu_count() or 1
+    per_traj = max(1, fired_local // n_traj) * M
+    sub = int(max(cores, min(n_traj, 1e9 // per_traj)))
+    t0 = time.perf_counter()
+    o = oracle.ensemble(net, x0, seed, traj0, sub, firings, t_end, n_threads=cores)
+    dt = time.perf_counter() - t0
+    return {"value": float(o["firings"].sum()) / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"trajectories {traj0}..{traj0 + sub - 1} of {workload} in full, {dt:.1f} s, "
+                      "one oracle instance per core"}
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2103_00405_b200 as rt
+
+    rt.lib()                                   # no extension -> ImportError; there is no fallback
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    head = measure(rt, torch, dist, args, args.workload, args.steps, args.warmup, rank, world, local, True)
+    secondary = {}
+    if args.secondary and world == 1 and args.scale == 1.0:
+        # the other configs of BASELINE.json, each timed exactly like the headline (fewer steps)
+        for wl in SECONDARY:
+            if wl == args.workload:
+                continue
+            s = measure(rt, torch, dist, args, wl, SECONDARY_STEPS, 3, rank, world, local, False)
+            s.pop("_cpu", None)
+            s["unit"] = UNIT if s["config"]["trajectories_per_step"] == 1 else "trajectory-steps/s"
+            s["steps"] = SECONDARY_STEPS
+            secondary[wl] = s
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": head["ms_per_step"],
+            "higher_is_better": True, "scaling": head["scaling"], "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": head["config"], "e2e": head["e2e"],
+            "gpu_launches": head["gpu_launches"], "clocks": head["clocks"], "roofline": head["roofline"],
+        }
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline(args.workload, *head["_cpu"])
+        if secondary:
+            line["secondary"] = secondary
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 

@@ -174,6 +174,21 @@ int rt_sync(rt_model *m, void *stream);
 int rt_set_rate_schedule(rt_model *m, int32_t n_break, const double *t_break, const double *factor,
                          const uint8_t *mask);
 
+/* Smoothly time-dependent rates (section 6, Eq.28, :224-231, the case the paper means by
+ * "the integral can be calculated analytically for well behaved time-dependent reaction rates"):
+ *   c_k(s) = c_k * exp(lambda[k] * s),   lambda [M] finite (decay < 0, growth > 0, 0 = constant).
+ * Every channel solves its own equation of Eq.28 in closed form each firing: with a_k(t) =
+ * c_k h_k exp(lambda_k t) the propensity now,
+ *   dt_k = log1p(lambda_k (P_k - T_k) / a_k(t)) / lambda_k     (+inf if the argument is <= -1),
+ *   T_k += a_k(t) * expm1(lambda_k dt_min) / lambda_k           for every k,
+ * and lambda_k = 0 takes the constant-rate formulas, so an all-zero lambda is the default path.
+ * exp / log1p / expm1 are the CUDA math library's (<= 2 ulp), so sample paths agree with a host
+ * implementation in the fired sequence and to ~1e-12 in the times, not to the last bit.
+ * lambda == NULL removes it; the array is copied.  Applies to rt_run / rt_run_resume /
+ * rt_ensemble (bundle kernel); not combinable with a rate schedule, "refresh_mode" = 1 or
+ * "formulation" = 1 (RT_ERR_UNSUPPORTED at run time).  RT_ERR_BAD_ARG for a non-finite lambda. */
+int rt_set_rate_exponent(rt_model *m, const double *lambda);
+
 /* Tuning / debug knobs (all optional; results never depend on them, except "formulation").
  *   "refresh_mode"   0 = dependency-graph refresh of a_k (default), 1 = recompute every a_k
  *                    each firing (the paper's own GPU scheme)

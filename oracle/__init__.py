@@ -28,6 +28,7 @@ def lib():
         _lib.oracle_binom.argtypes = [C.c_int64, C.c_int32]
         _lib.oracle_run.restype = C.c_int
         _lib.oracle_run_from.restype = C.c_int
+        _lib.oracle_run_rate_exp.restype = C.c_int
         _lib.oracle_run_residual.restype = C.c_int
         _lib.oracle_run_sched.restype = C.c_int
         _lib.oracle_ensemble.restype = C.c_int
@@ -174,6 +175,36 @@ def run_sched(net, x0, seed, trajectory=0, max_firings=0, t_end=math.inf, trace_
                                 _p(tmu, C.c_int32), _p(tt, C.c_double), C.c_uint64(trace_cap))
     if rc != 0:
         raise RuntimeError(f"oracle_run_sched failed with code {rc}")
+    nrec = min(int(firings.value), trace_cap)
+    return dict(x=x, t=t.value, firings=int(firings.value), stop=int(stop.value), fire_count=fc, T=T, P=P,
+                trace_mu=None if tmu is None else tmu[:nrec],
+                trace_t=None if tt is None else tt[:nrec])
+
+
+def run_rate_exp(net, x0, lam, seed, trajectory=0, max_firings=0, t_end=math.inf, trace_cap=0):
+    """One trajectory with smoothly time-dependent rates c_k(t) = c_k exp(lam[k] t) (PAPER.md
+    Eq.28 solved per channel in closed form)."""
+    args, keep = _net_args(net)
+    N, M = int(net["n_species"]), int(net["n_reactions"])
+    x0 = np.ascontiguousarray(x0, dtype=np.int64)
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    assert lam.shape == (M,)
+    x = np.zeros(N, dtype=np.int64)
+    t = C.c_double(0.0)
+    firings = C.c_uint64(0)
+    stop = C.c_int32(0)
+    fc = np.zeros(M, dtype=np.uint64)
+    T = np.zeros(M, dtype=np.float64)
+    P = np.zeros(M, dtype=np.float64)
+    tmu = np.zeros(trace_cap, dtype=np.int32) if trace_cap else None
+    tt = np.zeros(trace_cap, dtype=np.float64) if trace_cap else None
+    rc = lib().oracle_run_rate_exp(*args, _p(x0, C.c_int64), _p(lam, C.c_double), C.c_uint64(seed),
+                                   C.c_uint64(trajectory), C.c_uint64(max_firings), C.c_double(t_end),
+                                   _p(x, C.c_int64), C.byref(t), C.byref(firings), C.byref(stop),
+                                   _p(fc, C.c_uint64), _p(T, C.c_double), _p(P, C.c_double),
+                                   _p(tmu, C.c_int32), _p(tt, C.c_double), C.c_uint64(trace_cap))
+    if rc != 0:
+        raise RuntimeError(f"oracle_run_rate_exp failed with code {rc}")
     nrec = min(int(firings.value), trace_cap)
     return dict(x=x, t=t.value, firings=int(firings.value), stop=int(stop.value), fire_count=fc, T=T, P=P,
                 trace_mu=None if tmu is None else tmu[:nrec],

@@ -26,6 +26,7 @@
 //                    Table 2 (the NRRTA listing) lost its body in PAPER.md:258-260; the
 //                    (T_k, P_k) bookkeeping is reading G3 of DESIGN.md.
 //   nrrta_run_sched()     Eq.28 with piecewise-constant c_k(t)
+//   nrrta_run_rate_exp()  Eq.28 with c_k(t) = c_k exp(lambda_k t), solved per channel
 //   nrrta_run_residual()  Table 3 in residual-internal-time form (reading G4)
 //   Start / oracle_run_from()  the same two loops started from a checkpoint (t, T, P or R, n)
 //                    instead of step 0 -- no arithmetic of its own; pinned by the prefix identity
@@ -410,6 +411,114 @@ int nrrta_run_sched(const Net &net, const int64_t *x0, uint64_t seed, uint64_t t
   return rc;
 }
 
+// ---------------------------------------------------------------- smooth time-dependent rates
+// PAPER.md section 6, Eq.28 (:224-231) with a rate that varies smoothly in time, the case the paper
+// means by "the integral can be calculated analytically for well behaved time-dependent reaction
+// rates" (:229): the exponential family c_k(s) = c_k * exp(lambda_k * s), per-channel lambda_k
+// (decay < 0, growth > 0, 0 = constant).  With h_k = prod_j C(X_j, sigma_jk) constant between
+// firings and a_k(t) = c_k h_k exp(lambda_k t) the propensity at the start of the step,
+//     int_t^{t+d} c_k(s) h_k ds = a_k(t) * (exp(lambda_k d) - 1) / lambda_k,
+// so channel k's own equation of Eq.28, P_k - T_k = that integral, has the closed-form solution
+//     dt_k = log1p(lambda_k (P_k - T_k) / a_k(t)) / lambda_k,
+// which is +inf when lambda_k (P_k - T_k) / a_k(t) <= -1 (a decaying channel whose whole remaining
+// integral a_k(t)/|lambda_k| is smaller than its residual never fires again), and the internal
+// clocks advance by T_k += a_k(t) * (expm1(lambda_k d) / lambda_k)  (Eq.15 with Eq.1 inside).
+// lambda_k = 0 takes the constant-rate formulas of nrrta_run literally, so a run with every
+// lambda_k = 0 is nrrta_run bit for bit.  Operation order, each step one rounded operation:
+//     b_k = c_k * prod binom (as propensity());  g = exp(lambda_k * t);  a = b_k * g;
+//     x = (lambda_k * r) / a;  dt_k = log1p(x) / lambda_k;
+//     e = expm1(lambda_k * d) / lambda_k;  T_k = T_k + a * e.
+int nrrta_run_rate_exp(const Net &net, const int64_t *x0, const double *lambda, const Start *start,
+                       uint64_t seed, uint64_t traj, uint64_t max_firings, double t_end,
+                       int64_t *x_out, double *t_out, uint64_t *firings_out, int32_t *stop_out,
+                       uint64_t *fire_count_out, double *T_out, double *P_out,
+                       int32_t *trace_mu, double *trace_t, uint64_t trace_cap) {
+  const int32_t M = net.M, N = net.N;
+  const double INF = std::numeric_limits<double>::infinity();
+  const int64_t xmax = count_bound(net);
+  for (int64_t e = 0; e < net.react_ptr[M]; ++e)
+    if (net.react_sigma[e] < 1 || net.react_sigma[e] > 3) return ERR_BAD;
+  for (int32_t k = 0; k < M; ++k) if (!std::isfinite(lambda[k])) return ERR_BAD;
+  std::vector<int64_t> X(x0, x0 + N);
+  for (int32_t j = 0; j < N; ++j) if (X[j] < 0 || X[j] > xmax) return ERR_BAD;
+  std::vector<double> T(M, 0.0), P(M), a(M), dt(M);
+  std::vector<uint32_t> n(M, 0u);
+  for (int32_t k = 0; k < M; ++k) P[k] = exp_draw(seed, traj, (uint32_t)k, 0u);
+  double t = 0.0;
+  if (start) {
+    t = start->t;
+    if (start->T) for (int32_t k = 0; k < M; ++k) T[k] = start->T[k];
+    if (start->P) for (int32_t k = 0; k < M; ++k) P[k] = start->P[k];
+    if (start->n) for (int32_t k = 0; k < M; ++k) n[k] = (uint32_t)start->n[k];
+  }
+  uint64_t fired = 0;
+  int32_t stop = 0;
+  int rc = OK;
+  // T_k += int_t^{t+d} a_k(s) ds for every k, a[] = propensities at the start t of the interval
+  auto advance = [&](double d) {
+    for (int32_t k = 0; k < M; ++k) {
+      double e = d;
+      if (lambda[k] != 0.0) { const double ld = lambda[k] * d; e = std::expm1(ld) / lambda[k]; }
+      const double inc = a[k] * e;
+      T[k] = T[k] + inc;
+    }
+  };
+  for (;;) {
+    // step 1: instantaneous propensities a_k(t) = c_k h_k exp(lambda_k t)
+    for (int32_t k = 0; k < M; ++k) {
+      a[k] = propensity(net, X.data(), k);
+      if (lambda[k] != 0.0) { const double lt = lambda[k] * t; a[k] = a[k] * std::exp(lt); }
+    }
+    // step 2: each channel's own solution of Eq.28
+    for (int32_t k = 0; k < M; ++k) {
+      if (a[k] > 0.0) {
+        double r = P[k] - T[k];
+        if (r < 0.0) r = 0.0;
+        if (lambda[k] != 0.0) {
+          const double lr = lambda[k] * r;
+          const double x = lr / a[k];
+          dt[k] = (x > -1.0) ? std::log1p(x) / lambda[k] : INF;
+        } else {
+          dt[k] = r / a[k];
+        }
+      } else {
+        dt[k] = INF;
+      }
+    }
+    int32_t mu = 0;
+    double delta = dt[0];
+    for (int32_t k = 1; k < M; ++k)
+      if (dt[k] < delta) { delta = dt[k]; mu = k; }
+    if (delta == INF) { stop = STOP_ABSORBED; break; }
+    if (t_end < INF && t + delta > t_end) {
+      advance(t_end - t);
+      t = t_end;
+      stop = STOP_T_END;
+      break;
+    }
+    advance(delta);
+    t = t + delta;
+    rc = apply_firing(net, X.data(), mu, xmax);
+    n[mu] += 1u;
+    P[mu] = P[mu] + exp_draw(seed, traj, (uint32_t)mu, n[mu]);
+    if (fired < trace_cap) {
+      if (trace_mu) trace_mu[fired] = mu;
+      if (trace_t) trace_t[fired] = t;
+    }
+    fired += 1;
+    if (rc != OK) break;
+    if (max_firings != 0 && fired == max_firings) { stop = STOP_MAX_FIRINGS; break; }
+  }
+  if (x_out) for (int32_t j = 0; j < N; ++j) x_out[j] = X[j];
+  if (t_out) *t_out = t;
+  if (firings_out) *firings_out = fired;
+  if (stop_out) *stop_out = stop;
+  if (fire_count_out) for (int32_t k = 0; k < M; ++k) fire_count_out[k] = n[k];
+  if (T_out) for (int32_t k = 0; k < M; ++k) T_out[k] = T[k];
+  if (P_out) for (int32_t k = 0; k < M; ++k) P_out[k] = P[k];
+  return rc;
+}
+
 }  // namespace
 
 extern "C" {
@@ -476,6 +585,20 @@ int oracle_run_sched(int32_t N, int32_t M, const int64_t *react_ptr, const int32
   return nrrta_run_sched(net, x0, seed, traj, max_firings, t_end, n_break, t_break, factor, mask,
                          x_out, t_out, firings_out, stop_out, fire_count_out, T_out, P_out,
                          trace_mu, trace_t, trace_cap);
+}
+
+int oracle_run_rate_exp(int32_t N, int32_t M, const int64_t *react_ptr, const int32_t *react_species,
+                        const int32_t *react_sigma, const int64_t *stoich_ptr,
+                        const int32_t *stoich_species, const int32_t *stoich_v, const double *rate,
+                        const int64_t *x0, const double *lambda, uint64_t seed, uint64_t traj,
+                        uint64_t max_firings, double t_end, int64_t *x_out, double *t_out,
+                        uint64_t *firings_out, int32_t *stop_out, uint64_t *fire_count_out,
+                        double *T_out, double *P_out, int32_t *trace_mu, double *trace_t,
+                        uint64_t trace_cap) {
+  Net net{N, M, react_ptr, react_species, react_sigma, stoich_ptr, stoich_species, stoich_v, rate};
+  return nrrta_run_rate_exp(net, x0, lambda, nullptr, seed, traj, max_firings, t_end, x_out, t_out,
+                            firings_out, stop_out, fire_count_out, T_out, P_out, trace_mu, trace_t,
+                            trace_cap);
 }
 
 int oracle_run_residual(int32_t N, int32_t M, const int64_t *react_ptr, const int32_t *react_species,

@@ -10,7 +10,8 @@ from .binding import (  # noqa: F401
     RT_ERR_CUDA, RT_ERR_OOM, RT_STOP_T_END, RT_STOP_MAX_FIRINGS, RT_STOP_ABSORBED,
     RESULT_DTYPE, RtError, Model, lib, library_path,
     rt_validate_network, rt_create, rt_run, rt_run_resume, rt_run_dev, rt_ensemble, rt_ensemble_dev, rt_sync,
-    rt_set_option, rt_set_rate_schedule, rt_get_info, rt_destroy, rt_strerror,
+    rt_set_option, rt_set_rate_schedule, rt_set_rate_exponent, rt_get_info, rt_destroy, rt_strerror,
 )
 from .dist import shard_range, ensemble_sharded  # noqa: F401
 from .model_file import parse_model, load_model, ModelFileError  # noqa: F401
+from .rewrite import rewrite_trimolecular, RewriteError  # noqa: F401

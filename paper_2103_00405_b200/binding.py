@@ -60,6 +60,7 @@ def lib():
     L.rt_ensemble_dev.argtypes = [vp, vp, u64, u64, u64, u64, f64, vp, vp, vp]
     L.rt_sync.argtypes = [vp, vp]
     L.rt_set_rate_schedule.argtypes = [vp, C.c_int32, vp, vp, vp]
+    L.rt_set_rate_exponent.argtypes = [vp, vp]
     L.rt_set_option.argtypes = [vp, C.c_char_p, i64]
     L.rt_get_info.argtypes = [vp, C.c_char_p, C.POINTER(i64)]
     L.rt_destroy.argtypes = [vp]
@@ -67,6 +68,7 @@ def lib():
     L.rt_strerror.argtypes = [i32]
     L.rt_strerror.restype = C.c_char_p
     for name in ("rt_validate_network", "rt_create", "rt_run", "rt_run_resume", "rt_run_dev", "rt_ensemble", "rt_set_rate_schedule",
+                 "rt_set_rate_exponent",
                  "rt_ensemble_dev", "rt_sync", "rt_set_option", "rt_get_info"):
         getattr(L, name).restype = i32
     _lib = L
@@ -121,6 +123,16 @@ def rt_set_rate_schedule(handle, t_break, factor, mask=None):
     mk = None if mask is None else _np(mask, np.uint8)
     return lib().rt_set_rate_schedule(C.c_void_p(handle), int(tb.size), _ptr(tb) if tb.size else None,
                                       _ptr(fa) if fa.size else None, _ptr(mk))
+
+
+def rt_set_rate_exponent(handle, lam, n_reactions):
+    """c_k(t) = c_k exp(lam[k] t) (include/rt.h); lam = None removes it."""
+    if lam is None:
+        return lib().rt_set_rate_exponent(C.c_void_p(handle), None)
+    lam = _np(lam, np.float64)
+    if lam.shape != (n_reactions,):
+        return RT_ERR_BAD_ARG
+    return lib().rt_set_rate_exponent(C.c_void_p(handle), _ptr(lam))
 
 
 def rt_set_option(handle, name, value):
@@ -255,6 +267,11 @@ class Model:
         rc = rt_set_rate_schedule(self.handle, t_break, factor, mask)
         if rc != RT_OK:
             raise RtError(rc, "rt_set_rate_schedule")
+
+    def set_rate_exponent(self, lam):
+        rc = rt_set_rate_exponent(self.handle, lam, self.n_reactions)
+        if rc != RT_OK:
+            raise RtError(rc, "rt_set_rate_exponent")
 
     def info(self, name):
         return rt_get_info(self.handle, name)

@@ -79,7 +79,8 @@ struct rt_model {
   // per-bundle state
   DevBuf d_T, d_P, d_a, d_n, d_X, d_exch, d_err;
   // rate schedule (time-dependent rates)
-  DevBuf d_sched_t, d_sched_f, d_sched_mask;
+  DevBuf d_sched_t, d_sched_f, d_sched_mask, d_lambda;
+  bool rate_exp = false;     // exponential rates c_k exp(lambda_k t) are set
   int sched_n = 0;
   bool sched_has_mask = false;
   // staging for the host-pointer API
@@ -234,6 +235,8 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.prefetch = m->opt_prefetch;
   p.formulation = m->opt_formulation;
   if (m->sched_n > 0 && (m->refresh_mode != 0 || m->opt_formulation != 0 || start.T0)) return RT_ERR_UNSUPPORTED;
+  if (m->rate_exp && (m->refresh_mode != 0 || m->opt_formulation != 0 || m->sched_n > 0)) return RT_ERR_UNSUPPORTED;
+  p.rate_lambda = (const double *)m->d_lambda.p;
   p.sched_n = m->sched_n;
   p.sched_t = (const double *)m->d_sched_t.p;
   p.sched_f = (const double *)m->d_sched_f.p;
@@ -242,13 +245,15 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   void *args[] = {&p};
   // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
   const void *kern;
-  const bool sched = m->sched_n > 0;       // (never together with refresh_mode 1: checked above)
-  if (pl.smem) kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlockSmem, true, true, false>
-                      : sched         ? (const void *)rt::rt_bundle_kernel<kBlockSmem, true, false, true>
-                                      : (const void *)rt::rt_bundle_kernel<kBlockSmem, true, false, false>;
-  else kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, true, false>
-              : sched         ? (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, false, true>
-                              : (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, false, false>;
+  const int rate = m->sched_n > 0 ? 1 : m->rate_exp ? 2 : 0;   // (never with refresh_mode 1: checked above)
+  if (pl.smem) kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlockSmem, true, true, 0>
+                      : rate == 1     ? (const void *)rt::rt_bundle_kernel<kBlockSmem, true, false, 1>
+                      : rate == 2     ? (const void *)rt::rt_bundle_kernel<kBlockSmem, true, false, 2>
+                                      : (const void *)rt::rt_bundle_kernel<kBlockSmem, true, false, 0>;
+  else kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, true, 0>
+              : rate == 1     ? (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, false, 1>
+              : rate == 2     ? (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, false, 2>
+                              : (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, false, 0>;
   const size_t dyn = pl.smem ? smem_state_bytes(pl.pairs_per_cta) : 0;
   if (dyn) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
   // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
@@ -508,7 +513,8 @@ static int run_host(rt_model *m, const int64_t *x0, bool resume, double t0, cons
   // one-thread-per-trajectory kernel (which records no trace)
   const bool threads = resume && m->opt_ensemble_path == 1;
   if (threads) {
-    if (!thread_path_fits(m) || m->opt_formulation != 0 || m->sched_n > 0 || trace_cap) return RT_ERR_UNSUPPORTED;
+    if (!thread_path_fits(m) || m->opt_formulation != 0 || m->sched_n > 0 || m->rate_exp || trace_cap)
+      return RT_ERR_UNSUPPORTED;
     const Plan pl = plan_bundles(m, 1);
     if ((rc = ensure_state(m, pl)) != RT_OK) return rc;
     rc = launch_threads(m, (const long long *)m->d_x0.p, seed, trajectory, 1, max_firings, t_end,
@@ -563,11 +569,11 @@ int rt_ensemble_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t 
   if (n_traj == 0) return RT_OK;
   CU_TRY(cudaSetDevice(m->device));
   // (the thread kernel implements the plain (T,P) form with constant rates only)
-  bool use_threads = thread_path_fits(m) && m->opt_formulation == 0 && m->sched_n == 0;
+  bool use_threads = thread_path_fits(m) && m->opt_formulation == 0 && m->sched_n == 0 && !m->rate_exp;
   if (m->opt_ensemble_path == 1) {
     if (!thread_path_fits(m)) return RT_ERR_BAD_ARG;
     // the thread kernel implements the plain (T,P) form with constant rates only
-    if (m->opt_formulation != 0 || m->sched_n > 0) return RT_ERR_UNSUPPORTED;
+    if (m->opt_formulation != 0 || m->sched_n > 0 || m->rate_exp) return RT_ERR_UNSUPPORTED;
     use_threads = true;
   } else if (m->opt_ensemble_path == 2) {
     use_threads = false;
@@ -633,6 +639,24 @@ int rt_set_rate_schedule(rt_model *m, int32_t n_break, const double *t_break, co
   return RT_OK;
 }
 
+int rt_set_rate_exponent(rt_model *m, const double *lambda) {
+  if (!m) return RT_ERR_NULL;
+  if (!lambda) { m->rate_exp = false; return RT_OK; }
+  const size_t M = (size_t)m->net.M;
+  std::vector<double> lam((size_t)m->net.M_pad, 0.0);
+  bool any = false;
+  for (size_t k = 0; k < M; ++k) {
+    if (!std::isfinite(lambda[k])) return RT_ERR_BAD_ARG;
+    lam[k] = lambda[k];
+    any = any || lambda[k] != 0.0;
+  }
+  CU_TRY(cudaSetDevice(m->device));
+  int rc = upload(m->d_lambda, lam);
+  if (rc != RT_OK) return rc;
+  m->rate_exp = any;         // all zero: constant rates, the default kernel
+  return RT_OK;
+}
+
 int rt_set_option(rt_model *m, const char *name, int64_t value) {
   if (!m || !name) return RT_ERR_NULL;
   if (!strcmp(name, "refresh_mode")) {
@@ -687,7 +711,7 @@ void rt_destroy(rt_model *m) {
                     &m->d_T, &m->d_P, &m->d_a, &m->d_n, &m->d_X, &m->d_exch, &m->d_err,
                     &m->d_x0, &m->d_xout, &m->d_res, &m->d_trace_mu, &m->d_trace_t,
                     &m->d_T0, &m->d_P0, &m->d_n0,
-                    &m->d_sched_t, &m->d_sched_f, &m->d_sched_mask};
+                    &m->d_sched_t, &m->d_sched_f, &m->d_sched_mask, &m->d_lambda};
   for (DevBuf *b : bufs) b->release();
   delete m;
 }

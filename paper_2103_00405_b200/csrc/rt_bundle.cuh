@@ -71,6 +71,8 @@ struct BundleParams {
   int sched_n;
   const double *sched_t, *sched_f;
   const unsigned char *sched_mask;
+  // smoothly time-dependent rates (Eq.28): c_k(t) = c_k exp(rate_lambda[k] t), [M_pad]
+  const double *rate_lambda;
   int *err;               // set to 1 on a barrier timeout
 };
 
@@ -114,6 +116,40 @@ __device__ __forceinline__ double rcp_approx(double x) {
 __device__ __forceinline__ bool filter_unsafe(double a) {
   const unsigned ea = ((unsigned)__double2hiint(a) >> 20) & 0x7ffu;
   return (ea - 100u >= 1847u) && ((__double_as_longlong(a) << 1) != 0ll);
+}
+
+// ---- smooth time-dependent rates (Eq.28, :224-231): c_k(s) = c_k exp(lambda_k s) -------
+// The stored a_k is the time-independent part b_k = c_k h_k; the propensity at time t is
+// a_k(t) = b_k exp(lambda_k t).  Channel k's own equation of Eq.28,
+//   P_k - T_k = int_t^{t+d} a_k(s) ds = a_k(t) (exp(lambda_k d) - 1) / lambda_k,
+// is solved in closed form, dt_k = log1p(lambda_k (P_k - T_k) / a_k(t)) / lambda_k (+inf when the
+// argument is <= -1: a decaying channel whose remaining integral is smaller than its residual),
+// and the clocks advance by T_k += a_k(t) expm1(lambda_k d) / lambda_k.  lambda_k = 0 is the
+// constant-rate formula.  One rounded operation per step, in the order DESIGN.md fixes.
+struct RateExp {
+  const double *lam;     // [M_pad] lambda_k (0 in the padding)
+  double t_now;          // real time now (start of the interval being searched)
+  double t_prev;         // real time at the start of the interval that just elapsed (length dprev)
+};
+__device__ __noinline__ double waiting_time_exp(double P, double T, double b, double lam, double t) {
+  const double INF = __longlong_as_double(0x7ff0000000000000ll);
+  if (lam == 0.0) return waiting_time(P, T, b);
+  const double a = __dmul_rn(b, exp(__dmul_rn(lam, t)));
+  if (!(a > 0.0)) return INF;
+  double r = __dsub_rn(P, T);
+  r = r < 0.0 ? 0.0 : r;
+  const double x = __ddiv_rn(__dmul_rn(lam, r), a);
+  return x > -1.0 ? __ddiv_rn(log1p(x), lam) : INF;
+}
+__device__ __noinline__ double advance_exp(double T, double b, double lam, double t0, double d) {
+  if (lam == 0.0) return __dadd_rn(T, __dmul_rn(b, d));
+  const double a = __dmul_rn(b, exp(__dmul_rn(lam, t0)));
+  const double e = __ddiv_rn(expm1(__dmul_rn(lam, d)), lam);
+  return __dadd_rn(T, __dmul_rn(a, e));
+}
+template <bool EXPR>
+__device__ __forceinline__ double wt(double P, double T, double a, int k, const RateExp &rx) {
+  return EXPR ? waiting_time_exp(P, T, a, __ldg(rx.lam + k), rx.t_now) : waiting_time(P, T, a);
 }
 
 template <int NT, bool UPDATE>
@@ -248,16 +284,18 @@ __device__ __forceinline__ Cand scan_filtered_global(int tid, int k0, int k1, do
 // internal-time increment T_k += a_k * dprev (first pass); otherwise read-only (re-scan).
 // FULL: recompute a_k from X for every k (refresh_mode 1).
 // Ownership: STATE_SMEM -- local index i = tid, tid+NT, ...; global state -- pair q0+tid, +NT, ...
-template <int NT, bool SMEM, bool UPDATE>
+// EXPR: exponential time-dependent rates (plain loops with the closed-form solve; no filter).
+template <int NT, bool SMEM, bool UPDATE, bool EXPR = false>
 __device__ __forceinline__ Cand scan_own(const NetDev &net, const u64 *X, int tid, int k0, int k1,
                                          double *sT, const double *sP, double *sA,
                                          double *T, double *P, double *A, double dprev, bool full,
-                                         int cnt_pad, bool any_odd, bool &defer, bool resid = false) {
+                                         int cnt_pad, bool any_odd, bool &defer, bool resid = false,
+                                         const RateExp &rx = RateExp()) {
   Cand best;
   best.dt = __longlong_as_double(0x7ff0000000000000ll);
   best.k = 0x7fffffff;
-  if (SMEM && !full) return scan_filtered<NT, UPDATE>(tid, k0, cnt_pad, sT, sP, sA, dprev, any_odd, defer);
-  if (!SMEM && !full)
+  if (!EXPR && SMEM && !full) return scan_filtered<NT, UPDATE>(tid, k0, cnt_pad, sT, sP, sA, dprev, any_odd, defer);
+  if (!EXPR && !SMEM && !full)
     return resid ? scan_filtered_global<NT, UPDATE, true>(tid, k0, k1, T, P, A, dprev, any_odd, defer)
                  : scan_filtered_global<NT, UPDATE, false>(tid, k0, k1, T, P, A, dprev, any_odd, defer);
   if (SMEM) {
@@ -267,14 +305,14 @@ __device__ __forceinline__ Cand scan_own(const NetDev &net, const u64 *X, int ti
       double a = sA[i], t = sT[i];
       const double pk = sP[i];
       if (UPDATE) {
-        t = __dadd_rn(t, __dmul_rn(a, dprev));
+        t = EXPR ? advance_exp(t, a, __ldg(rx.lam + k0 + i), rx.t_prev, dprev) : __dadd_rn(t, __dmul_rn(a, dprev));
         sT[i] = t;
         if (full) {
           a = (k0 + i < net.M) ? propensity(net, X, k0 + i) : 0.0;
           sA[i] = a;
         }
       }
-      const double d = waiting_time(pk, t, a);
+      const double d = wt<EXPR>(pk, t, a, k0 + i, rx);
       if (d < best.dt) { best.dt = d; best.k = k0 + i; }
     }
   } else {
@@ -297,8 +335,13 @@ __device__ __forceinline__ Cand scan_own(const NetDev &net, const u64 *X, int ti
       for (int u = 0; u < U; ++u) {
         const int qu = q + u * NT;
         if (UPDATE && qu < q1) {
-          tt[u].x = __dadd_rn(tt[u].x, __dmul_rn(aa[u].x, dprev));
-          tt[u].y = __dadd_rn(tt[u].y, __dmul_rn(aa[u].y, dprev));
+          if (EXPR) {
+            tt[u].x = advance_exp(tt[u].x, aa[u].x, __ldg(rx.lam + 2 * qu), rx.t_prev, dprev);
+            tt[u].y = advance_exp(tt[u].y, aa[u].y, __ldg(rx.lam + 2 * qu + 1), rx.t_prev, dprev);
+          } else {
+            tt[u].x = __dadd_rn(tt[u].x, __dmul_rn(aa[u].x, dprev));
+            tt[u].y = __dadd_rn(tt[u].y, __dmul_rn(aa[u].y, dprev));
+          }
           __stcg(T2 + qu, tt[u]);
           if (full) {
             aa[u].x = (2 * qu < net.M) ? propensity(net, X, 2 * qu) : 0.0;
@@ -306,9 +349,9 @@ __device__ __forceinline__ Cand scan_own(const NetDev &net, const u64 *X, int ti
             __stcg(A2 + qu, aa[u]);
           }
         }
-        double d = waiting_time(pp[u].x, tt[u].x, aa[u].x);
+        double d = (qu < q1) ? wt<EXPR>(pp[u].x, tt[u].x, aa[u].x, 2 * qu, rx) : best.dt;
         if (d < best.dt) { best.dt = d; best.k = 2 * qu; }
-        d = waiting_time(pp[u].y, tt[u].y, aa[u].y);
+        d = (qu < q1) ? wt<EXPR>(pp[u].y, tt[u].y, aa[u].y, 2 * qu + 1, rx) : best.dt;
         if (d < best.dt) { best.dt = d; best.k = 2 * qu + 1; }
       }
     }
@@ -611,9 +654,11 @@ __device__ __noinline__ bool bundle_barrier(u64 *exch, int S, int r, uint32_t ge
 
 // FULL = refresh_mode 1 (recompute every a_k each firing, the paper's own GPU scheme) is a separate
 // instantiation so that its code stays out of the instruction stream of the default kernel.
-// SCHED = a rate schedule is set (time-dependent rates): also its own instantiation.
-template <int BLOCK, bool SMEM, bool FULL, bool SCHED>
+// RATE = 1: a piecewise-constant rate schedule is set; RATE = 2: exponential rates c_k exp(lambda_k t)
+// (time-dependent rates, Eq.28): also their own instantiations.
+template <int BLOCK, bool SMEM, bool FULL, int RATE>
 __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams p) {
+  constexpr bool SCHED = RATE == 1, EXPR = RATE == 2;
   constexpr int NT = BLOCK - 32 * kWalkerWarps;      // stream threads; the last warp walks
   __shared__ BundleCtx<BLOCK> ctx;
   __shared__ int list_k[kListCap];
@@ -694,6 +739,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     __syncthreads();
 
     double t = p.t0, dprev = 0.0;
+    RateExp rx;                          // (EXPR only)
+    rx.lam = p.rate_lambda; rx.t_now = t; rx.t_prev = t;
     u64 fired = 0;
     int mu_prev = -1, stop = 0, status = RT_OK;
     bool finishing = false;
@@ -873,8 +920,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         } else if (first_round) {
           // ===== stream warps: a-5 of the previous firing fused with a-2/a-3 of this one =====
           bool defer = false;
-          best = scan_own<NT, SMEM, true>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, dprev, full, cnt_pad,
-                                          ctx.any_odd != 0, defer, resid);
+          best = scan_own<NT, SMEM, true, EXPR>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, dprev, full, cnt_pad,
+                                                ctx.any_odd != 0, defer, resid, rx);
           mybest_k[tid] = defer ? -3 : best.k;
           if (defer) dirty[tid] = 1;
         }
@@ -896,8 +943,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           if (mybest_k[o] == k || mybest_k[o] == -3 || k == pk_now) {
             dirty[o] = 1;
           } else {
-            const double d = waiting_time(SMEM ? sP[k - k0] : __ldcg(P + k),
-                                          SMEM ? sT[k - k0] : __ldcg(T + k), a_new);
+            const double d = wt<EXPR>(SMEM ? sP[k - k0] : __ldcg(P + k),
+                                      SMEM ? sT[k - k0] : __ldcg(T + k), a_new, k, rx);
             if (cand_less(d, k, extra)) { extra.dt = d; extra.k = k; }
           }
         }
@@ -943,14 +990,14 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
               stale_mask &= stale_mask - 1;
               const int i = (tid - lane + L) + lane * NT;      // lane j: the thread's j-th reaction
               Cand c = none;
-              if (i < cnt_pad) { c.dt = waiting_time(sP[i], sT[i], sA[i]); c.k = k0 + i; }
+              if (i < cnt_pad) { c.dt = wt<EXPR>(sP[i], sT[i], sA[i], min(k0 + i, net.M_pad - 1), rx); c.k = k0 + i; }
               c = warp_lexmin(c);
               if (lane == L) best = c;
             }
           } else if (stale_mask & (1u << lane)) {
             bool defer = false;
-            best = scan_own<NT, SMEM, false>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, 0.0, false, cnt_pad,
-                                             ctx.any_odd != 0, defer);
+            best = scan_own<NT, SMEM, false, EXPR>(net, X, tid, k0, k1, sT, sP, sA, T, P, A, 0.0, false, cnt_pad,
+                                                   ctx.any_odd != 0, defer, false, rx);
           }
         }
       } else {
@@ -970,9 +1017,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
             Cand c = none;
             for (int q = (k0 >> 1) + d + lane * NT; q < (k1 >> 1); q += 32 * NT) {
               const double2 t2 = __ldcg(T2 + q), p2 = __ldcg(P2 + q), a2 = __ldcg(A2 + q);
-              double w = waiting_time(p2.x, t2.x, a2.x);
+              double w = wt<EXPR>(p2.x, t2.x, a2.x, 2 * q, rx);
               if (cand_less(w, 2 * q, c)) { c.dt = w; c.k = 2 * q; }
-              w = waiting_time(p2.y, t2.y, a2.y);
+              w = wt<EXPR>(p2.y, t2.y, a2.y, 2 * q + 1, rx);
               if (cand_less(w, 2 * q + 1, c)) { c.dt = w; c.k = 2 * q + 1; }
             }
             c = warp_lexmin(c);
@@ -1009,6 +1056,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       if (delta == INF) { stop = RT_STOP_ABSORBED; break; }
       if (p.t_end < INF && __dadd_rn(t, delta) > p.t_end) {
         dprev = __dsub_rn(p.t_end, t);           // closing pass: T_k += a_k * (t_end - t), no firing
+        rx.t_prev = t; rx.t_now = p.t_end;
         t = p.t_end;
         mu_prev = -1;
         stop = RT_STOP_T_END;
@@ -1016,7 +1064,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         continue;
       }
       if (fired >= kXMaxVersion) { status = RT_ERR_OVERFLOW; break; }   // firing counter exhausted
+      rx.t_prev = t;
       t = __dadd_rn(t, delta);
+      rx.t_now = t;
       fired += 1;
       mu_prev = win.k;
       dprev = delta;
