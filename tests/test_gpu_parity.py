@@ -678,9 +678,13 @@ def test_exponential_rates_decay_to_silence_hub_network_and_ensemble(rt):
     net, x0 = _hub_network()
     M = int(net["n_reactions"])
     o0 = _oracle().run(net, x0, 21, 0, 300, math.inf, 300)
-    lam = np.full(M, -1.0 / float(o0["trace_t"][200]))
+    # One common lambda < 0 is a time change of the constant-rate run: internal time saturates at
+    # 1/|lambda|, so the decaying run fires exactly the constant-rate firings before that instant.
+    # Put it BETWEEN two firings (on a firing time the last channel's argument is -1 +- rounding).
+    lam = np.full(M, -2.0 / float(o0["trace_t"][200] + o0["trace_t"][201]))
     g, o = _check_rate_exp(rt, net, x0, lam, 21, 0, 100000, math.inf, 4096)
-    assert g["stop"] == rt.RT_STOP_ABSORBED and 100 < g["firings"] < 100000
+    assert g["stop"] == rt.RT_STOP_ABSORBED and g["firings"] == 201
+    np.testing.assert_array_equal(g["trace_mu"][:201], o0["trace_mu"][:201])
     net, x0 = W.lotka_volterra(y1=60, y2=40, c1=2.0, c2=0.02, c3=1.5)
     lam3 = [0.4, -0.3, 0.0]
     with rt.Model(net) as m:
