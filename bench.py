@@ -308,6 +308,8 @@ def measure(rt, torch, dist, args, workload, steps, warmup, rank, world, local, 
             "l2": "flushed between steps (256 MB fill)",
             "bundle_ctas": model.info("bundle_ctas"), "bundles": model.info("bundles"),
             "block_threads": model.info("block_threads"), "state_in_shared_memory": smem,
+            "exchange": ("thread-block cluster (DSMEM)" if model.info("cluster_exchange") else
+                         "L2 slots" if model.info("bundle_ctas") > 1 else "none"),
             "us_per_firing": us_per_firing, "ensemble_path": model.info("ensemble_path"),
             "formulation": "residual (Table 3)" if formulation else "(T, P) internal time",
             "rate_breakpoints": breakpoints}

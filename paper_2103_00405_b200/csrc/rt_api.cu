@@ -87,6 +87,9 @@ struct rt_model {
   DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t, d_T0, d_P0, d_n0;
   // options
   int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0, opt_prefetch = 7, opt_formulation = 0;
+  int opt_exchange = 0;
+  int max_clusters[rt::kMaxClusterCtas + 1] = {};   // co-resident clusters per cluster size (0 = not asked yet, -1 = none)
+  int last_cluster = 0;
   // info
   int64_t kernel_launches = 0;
   int last_S = 0, last_B = 0, last_path = 0, last_state_smem = 0, last_block = 0;
@@ -159,7 +162,8 @@ struct StartDev {
 };
 
 // How one launch is shaped: B bundles of S CTAs; smem = the (T,P,a) state lives in shared memory.
-struct Plan { int S, B, G; int pairs_per_cta; int cnt_pad; bool smem; };
+// cluster = each bundle is one thread-block cluster and exchanges through distributed shared memory.
+struct Plan { int S, B, G; int pairs_per_cta; int cnt_pad; bool smem; bool cluster; };
 
 // slots per shared-memory state array: a CTA's reactions padded to whole scan batches
 int padded_count(int pairs_per_cta) {
@@ -168,7 +172,50 @@ int padded_count(int pairs_per_cta) {
 }
 size_t smem_state_bytes(int pairs_per_cta) { return (size_t)padded_count(pairs_per_cta) * 3 * sizeof(double); }
 
-Plan plan_bundles(const rt_model *m, u64 n_traj) {
+// The bundle kernel for a launch shape (FULL = refresh_mode 1; rate: 0 constant, 1 schedule, 2 exponential).
+const void *bundle_kernel(bool smem, bool full, int rate, bool cluster) {
+  using namespace rt;
+  if (smem && cluster)
+    return full        ? (const void *)rt_bundle_kernel<kBlockSmem, true, true, 0, true>
+           : rate == 1 ? (const void *)rt_bundle_kernel<kBlockSmem, true, false, 1, true>
+           : rate == 2 ? (const void *)rt_bundle_kernel<kBlockSmem, true, false, 2, true>
+                       : (const void *)rt_bundle_kernel<kBlockSmem, true, false, 0, true>;
+  if (smem)
+    return full        ? (const void *)rt_bundle_kernel<kBlockSmem, true, true, 0>
+           : rate == 1 ? (const void *)rt_bundle_kernel<kBlockSmem, true, false, 1>
+           : rate == 2 ? (const void *)rt_bundle_kernel<kBlockSmem, true, false, 2>
+                       : (const void *)rt_bundle_kernel<kBlockSmem, true, false, 0>;
+  return full        ? (const void *)rt_bundle_kernel<kBlockGlobal, false, true, 0>
+         : rate == 1 ? (const void *)rt_bundle_kernel<kBlockGlobal, false, false, 1>
+         : rate == 2 ? (const void *)rt_bundle_kernel<kBlockGlobal, false, false, 2>
+                     : (const void *)rt_bundle_kernel<kBlockGlobal, false, false, 0>;
+}
+
+// Clusters of S CTAs (one per SM: the state fills shared memory) that can be co-resident; the GPC
+// structure decides (B200: 74 of 2, 33 of 4, 15 of 8, 7 of 16).  Asked once per size.
+int max_active_clusters(rt_model *m, int S) {
+  if (S < 2 || S > rt::kMaxClusterCtas) return 0;
+  if (m->max_clusters[S] == 0) {
+    const void *kern = bundle_kernel(true, false, 0, true);
+    int n = 0;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(S); cfg.blockDim = dim3(kBlockSmem); cfg.dynamicSmemBytes = kSmemStateBytes;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = S; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemStateBytes) != cudaSuccess ||
+        cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess ||
+        cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) {
+      cudaGetLastError();
+      n = 0;
+    }
+    m->max_clusters[S] = n > 0 ? n : -1;
+  }
+  return std::max(m->max_clusters[S], 0);
+}
+
+Plan plan_bundles(rt_model *m, u64 n_traj) {
   const int pairs_total = m->net.M_pad / 2;
   const int sms = m->num_sms;
   // fewest CTAs whose share of the state still fits in shared memory
@@ -176,25 +223,49 @@ Plan plan_bundles(const rt_model *m, u64 n_traj) {
   const int pairs_fit = std::max(1, (int)(kSmemStateBytes / (3 * sizeof(double)) / batch * batch / 2));
   const int s_fit = (pairs_total + pairs_fit - 1) / pairs_fit;
   const int s_thin = std::max(1, (pairs_total + kMinPairsPerCta - 1) / kMinPairsPerCta);
-  int S;
+  const bool may_cluster = m->opt_exchange != 1 && m->opt_state_mode != 1;
+  int S, B = 0;
+  bool cluster = false;
   if (m->opt_bundle_ctas > 0) {
     S = std::min(m->opt_bundle_ctas, sms);
   } else if (n_traj <= 1) {
-    S = std::min(sms, s_thin);                          // one trajectory: the whole chip
+    S = std::min(sms, s_thin);                          // one trajectory: the whole chip ...
+    // ... unless ONE cluster holds the state: its exchange through distributed shared memory costs
+    // ~0.25 us instead of ~1.2 us through L2 (profiles/r2_exchange_floor.md), which outweighs the
+    // longer pass of fewer, fuller CTAs.
+    const int sc = std::min(rt::kMaxClusterCtas, s_thin);
+    if (may_cluster && sc >= 2 && sc >= s_fit && max_active_clusters(m, sc) >= 1) S = sc;
   } else {
     S = (int)std::max<u64>(1, (u64)sms / n_traj);       // many: as many bundles as fit ...
     if (m->opt_state_mode != 1 && S < s_fit && s_fit <= sms) S = s_fit;   // ... with on-chip state
     S = std::min(S, s_thin);
+    if (may_cluster && S >= 2 && S <= rt::kMaxClusterCtas && S >= s_fit) {
+      // cluster bundles: among the sizes from S up, the one with the best modelled throughput
+      // B(S) / (fixed per-firing latency + pass time), both ~1 us at 6250 reactions per CTA
+      double best = 0.0;
+      int best_S = 0;
+      for (int c = S; c <= std::min(rt::kMaxClusterCtas, s_thin); ++c) {
+        const int bc = (int)std::min<u64>(n_traj, (u64)max_active_clusters(m, c));
+        const double thr = bc / (1.0 + (double)pairs_total / c / 3125.0);
+        if (thr > best) { best = thr; best_S = c; }
+      }
+      if (best_S) S = best_S;
+    }
   }
   S = std::max(std::min(S, rt::kMaxBundleCtas), 1);
   Plan pl;
   pl.S = S;
-  pl.B = (int)std::min<u64>(std::max<u64>(n_traj, 1), (u64)(sms / S));
   pl.pairs_per_cta = (pairs_total + S - 1) / S;
-  pl.G = std::min(S, m->opt_x_replicas > 0 ? m->opt_x_replicas : 1);      // X replicas: spread the per-firing reads/atomics of hot species
-  while (pl.G > 1 && (size_t)pl.B * pl.G * (size_t)m->net.N * 8 > ((size_t)64 << 20)) pl.G /= 2;
   pl.cnt_pad = padded_count(pl.pairs_per_cta);
   pl.smem = m->opt_state_mode != 1 && smem_state_bytes(pl.pairs_per_cta) <= kSmemStateBytes;
+  if (may_cluster && pl.smem && S >= 2 && S <= rt::kMaxClusterCtas) {
+    B = (int)std::min<u64>(std::max<u64>(n_traj, 1), (u64)max_active_clusters(m, S));
+    cluster = B >= 1;
+  }
+  pl.cluster = cluster;
+  pl.B = cluster ? B : (int)std::min<u64>(std::max<u64>(n_traj, 1), (u64)(sms / S));
+  pl.G = std::min(S, m->opt_x_replicas > 0 ? m->opt_x_replicas : 1);      // X replicas: spread the per-firing reads/atomics of hot species
+  while (pl.G > 1 && (size_t)pl.B * pl.G * (size_t)m->net.N * 8 > ((size_t)64 << 20)) pl.G /= 2;
   return pl;
 }
 
@@ -243,25 +314,31 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.sched_mask = m->sched_has_mask ? (const unsigned char *)m->d_sched_mask.p : nullptr;
   p.err = (int *)m->d_err.p;
   void *args[] = {&p};
-  // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
-  const void *kern;
   const int rate = m->sched_n > 0 ? 1 : m->rate_exp ? 2 : 0;   // (never with refresh_mode 1: checked above)
-  if (pl.smem) kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlockSmem, true, true, 0>
-                      : rate == 1     ? (const void *)rt::rt_bundle_kernel<kBlockSmem, true, false, 1>
-                      : rate == 2     ? (const void *)rt::rt_bundle_kernel<kBlockSmem, true, false, 2>
-                                      : (const void *)rt::rt_bundle_kernel<kBlockSmem, true, false, 0>;
-  else kern = m->refresh_mode ? (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, true, 0>
-              : rate == 1     ? (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, false, 1>
-              : rate == 2     ? (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, false, 2>
-                              : (const void *)rt::rt_bundle_kernel<kBlockGlobal, false, false, 0>;
+  const void *kern = bundle_kernel(pl.smem, m->refresh_mode != 0, rate, pl.cluster);
   const size_t dyn = pl.smem ? smem_state_bytes(pl.pairs_per_cta) : 0;
   if (dyn) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-  // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
   const int block = pl.smem ? kBlockSmem : kBlockGlobal;
-  CU_TRY(cudaLaunchCooperativeKernel(kern, dim3(pl.S * pl.B), dim3(block), args, dyn, st));
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(pl.S * pl.B); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = dyn; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  if (pl.cluster) {
+    // One cluster per bundle: the hardware co-schedules its CTAs, and bundles never wait for one
+    // another, so no cooperative launch is needed.
+    if (pl.S > 8) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = pl.S; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  } else {
+    // Cooperative launch: the CTAs of a bundle spin on one another, so all must be co-resident.
+    at[0].id = cudaLaunchAttributeCooperative;
+    at[0].val.cooperative = 1;
+  }
+  cfg.attrs = at; cfg.numAttrs = 1;
+  CU_TRY(cudaLaunchKernelExC(&cfg, kern, args));
   m->last_block = block;
   m->kernel_launches += 1;
   m->last_S = pl.S; m->last_B = pl.B; m->last_path = 2; m->last_state_smem = pl.smem ? 1 : 0;
+  m->last_cluster = pl.cluster ? 1 : 0;
   return RT_OK;
 }
 
@@ -680,6 +757,9 @@ int rt_set_option(rt_model *m, const char *name, int64_t value) {
   } else if (!strcmp(name, "state_mode")) {
     if (value < 0 || value > 1) return RT_ERR_BAD_ARG;
     m->opt_state_mode = (int)value;
+  } else if (!strcmp(name, "exchange")) {
+    if (value < 0 || value > 1) return RT_ERR_BAD_ARG;
+    m->opt_exchange = (int)value;
   } else {
     return RT_ERR_BAD_ARG;
   }
@@ -697,6 +777,7 @@ int rt_get_info(const rt_model *m, const char *name, int64_t *value) {
   else if (!strcmp(name, "dep_entries")) *value = m->nnz_r;
   else if (!strcmp(name, "max_sigma")) *value = m->max_sigma;
   else if (!strcmp(name, "state_in_smem")) *value = m->last_state_smem;
+  else if (!strcmp(name, "cluster_exchange")) *value = m->last_cluster;
   else if (!strcmp(name, "hub_species")) *value = (int64_t)m->n_big;
   else return RT_ERR_BAD_ARG;
   return RT_OK;

@@ -90,6 +90,10 @@ struct BundleCtx {
   int n_stale;            // global-memory state: threads whose candidate must be re-scanned
   int p_k;                // reaction whose P was redrawn (or -1), and its new value
   double p_val;
+  // cluster bundles: every peer's (dt, k) lands here by st.async, double-buffered by generation
+  // parity; cl_bar[b] counts the 16 * S bytes of generation parity b
+  alignas(16) u64 cl_slot[2][kMaxClusterCtas][2];
+  alignas(8) u64 cl_bar[2];
 };
 
 // ---- filtered scan (state in shared memory) ----------------------------------------------------
@@ -499,22 +503,77 @@ struct Spec {
 // Block-wide lexmin of the thread candidates, then all-gather of the S CTA partials through the
 // exchange slots (which is also the per-firing bundle barrier).  Every thread returns the
 // bundle-wide winner.  win.k == -2 signals a timeout.
-template <int BLOCK, bool PREWALK>
+// Named barriers of the kernel: 0 = __syncthreads; 1 = the stream warps among themselves; 2 = warp 0
+// hands the winner to the walker warp; 3 = the walker's staged refreshes are ready (kBarStaged);
+// 4 = the stream warps' partials are ready for the walker (kBarParts).
+constexpr int kBarStaged = 3, kBarParts = 4;
+template <int COUNT> __device__ __forceinline__ void named_sync(int id) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(COUNT) : "memory");
+}
+template <int COUNT> __device__ __forceinline__ void named_arrive(int id) {
+  __threadfence_block();
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "n"(COUNT) : "memory");
+}
+
+// Pre-walk of the runner-up k2 (walker warp): row -> ranges -> this CTA's dependency entries, into
+// pw_d / pw_c.  Network data only, so it stays valid until another reaction is pre-walked.
+__device__ __forceinline__ void prewalk(const BundleParams &p, Spec &spec, int lane);
+
+// FREE: the walker warp runs ahead of the stream warps (see the kernel): it does not post a partial
+// and pre-walks BEFORE it waits for the stream warps' partials.
+template <int BLOCK, bool PREWALK, bool CLUSTER, bool FREE>
 __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<BLOCK> &ctx,
                                               u64 *exch, const uint32_t *nfire, int r,
                                               uint32_t &gen, Cand mine, Spec &spec) {
   constexpr int NT = BLOCK - 32 * kWalkerWarps;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  mine = warp_lexmin(mine);
-  if (lane == 0) ctx.warp_part[warp] = mine;
-  __syncthreads();
+  const bool walker = warp == BLOCK / 32 - 1;
+  if (!walker) {
+    mine = warp_lexmin(mine);
+    if (lane == 0) ctx.warp_part[warp] = mine;
+  }
+  if (FREE) {
+    if (walker) {
+      if (PREWALK && (p.prefetch & 4)) prewalk(p, spec, lane);
+      named_sync<BLOCK>(kBarParts);
+    } else {
+      named_sync<NT>(1);
+      named_arrive<BLOCK>(kBarParts);
+    }
+  } else {
+    __syncthreads();
+  }
   if (warp == 0) {
-    Cand c = ctx.warp_part[lane];                 // BLOCK / 32 <= 32 partials
-    if (lane >= BLOCK / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
+    Cand c = ctx.warp_part[lane];                 // NT / 32 <= 32 partials
+    if (lane >= NT / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
     c = warp_lexmin(c);
     Cand c2;                                      // this lane's second-best slot (runner-up search)
     c2.dt = __longlong_as_double(0x7ff0000000000000ll); c2.k = 0x7fffffff;
-    if (p.S > 1) {
+    if (CLUSTER && p.S > 1) {
+      // One thread-block cluster = one bundle: lane l stores this CTA's partial into slot r of
+      // peer l (st.async: the store also completes 16 bytes on the peer's mbarrier), then every
+      // CTA waits for its own 16 * S bytes.  No global memory on the path.
+      const uint32_t par = gen & 1u, ph = (gen >> 1) & 1u;
+      const uint32_t bar = smem_addr(&ctx.cl_bar[par]);
+      if (lane == 0) mbar_arrive_expect_tx(bar, 16u * (uint32_t)p.S);
+      if (lane < p.S)
+        st_async_v2(mapa_u32(smem_addr(&ctx.cl_slot[par][r][0]), (uint32_t)lane),
+                    (u64)__double_as_longlong(c.dt), (u64)(uint32_t)c.k, mapa_u32(bar, (uint32_t)lane));
+      const long long t0 = clock64();
+      bool timed_out = false;
+      while (!mbar_try_wait(bar, ph))
+        if (clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); timed_out = true; break; }
+      Cand s;
+      s.dt = __longlong_as_double(0x7ff0000000000000ll); s.k = 0x7fffffff;
+      if (lane < p.S) {
+        s.dt = __longlong_as_double((long long)ctx.cl_slot[par][lane][0]);
+        s.k = (int)(uint32_t)ctx.cl_slot[par][lane][1];
+      }
+      c = warp_lexmin(s);
+      if (s.k == c.k) { s.dt = __longlong_as_double(0x7ff0000000000000ll); s.k = 0x7fffffff; }
+      c2 = warp_lexmin(s);                        // runner-up: best of everything but the winner
+      if (__any_sync(0xffffffffu, timed_out)) c.k = -2;
+    } else if (p.S > 1) {
       const uint32_t tag = gen + 1u;
       const u64 par = (u64)(((gen >> 1) & 1u) ^ 1u) << 63;     // never matches zeroed memory
       u64 *buf = exch + (size_t)(gen & 1u) * (size_t)p.S * kSlotStride;
@@ -553,39 +612,16 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
       if (timed_out) c.k = -2;
     }
     if (lane == 0) { ctx.win = c; ctx.second_k = (c2.dt < __longlong_as_double(0x7ff0000000000000ll)) ? c2.k : 0x7fffffff; }
-  } else if (warp == BLOCK / 32 - 1) {
+  } else if (walker) {
     // Walker warp, idle during the exchange.  If this CTA's candidate wins (it usually stays the
     // candidate for many firings before it does), this CTA must redraw P_k (Philox + log, the
     // longest serial piece of a firing) and every CTA will need the candidate's stoich row and
     // the dependency entries of its species, all DRAM-cold (each reaction fires rarely).
     // Do the redraw now, speculatively, and pull the rest into L2 -- once per candidate.
     Cand c = ctx.warp_part[lane];
-    if (lane >= BLOCK / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
+    if (lane >= NT / 32) { c.dt = __longlong_as_double(0x7ff0000000000000ll); c.k = 0x7fffffff; }
     c = warp_lexmin(c);
-    if (PREWALK && (p.prefetch & 4) && spec.k2 != spec.pw_k && spec.k2 < p.net.M && spec.k1 > spec.k0) {
-      // pre-walk of the runner-up: row -> ranges -> this CTA's dependency entries, into pw_d / pw_c
-      const int k2 = spec.k2;
-      int4 ent = make_int4(-1, 0, 0, 0);
-      if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(p.net.srow) + (size_t)k2 * 4 + lane);
-      spec.pw_k = -1;
-      if (__shfl_sync(0xffffffffu, ent.x, 0) != -2) {
-        uint32_t lo = 0, hi = 0;
-        if (ent.x >= 0) { lo = (uint32_t)ent.z; hi = (uint32_t)ent.w; narrow_range(p.net, lo, hi, spec.k0, spec.k1); }
-        Ranges rg;
-        uint32_t acc = 0;
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          rg.lo[e] = __shfl_sync(0xffffffffu, lo, e);
-          acc += __shfl_sync(0xffffffffu, hi - lo, e);
-          rg.end[e] = acc;
-        }
-        uint32_t f = 0;
-        int n = 0;
-        if (!walk_scan(p.net, rg, f, spec.k0, spec.k1, lane, n, spec.pw_d, spec.pw_c)) {
-          spec.pw_k = k2; spec.pw_n = n; spec.pw_ent = ent;
-        }
-      }
-    }
+    if (!FREE && PREWALK && (p.prefetch & 4)) prewalk(p, spec, lane);
     if (c.k < p.net.M && c.k != spec.k && lane == 0 && (p.prefetch & 2)) {
       const uint32_t n1 = nfire[c.k] + 1u;
       if (p.formulation) {
@@ -616,18 +652,47 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
   // The stream warps leave as soon as warp 0 has the winner; the walker warp, which may still
   // be busy with its speculative work, pairs with warp 0 on a barrier of its own.
   if (warp == 0) asm volatile("bar.arrive 2, 64;" ::: "memory");
-  if (warp == BLOCK / 32 - 1) { asm volatile("bar.sync 2, 64;" ::: "memory"); spec.k2 = ctx.second_k; }
+  if (walker) { asm volatile("bar.sync 2, 64;" ::: "memory"); spec.k2 = ctx.second_k; }
   else asm volatile("bar.sync 1, %0;" ::"r"(NT) : "memory");
   return ctx.win;
+}
+
+__device__ __forceinline__ void prewalk(const BundleParams &p, Spec &spec, int lane) {
+  if (spec.k2 == spec.pw_k || spec.k2 >= p.net.M || spec.k1 <= spec.k0) return;
+  const int k2 = spec.k2;
+  int4 ent = make_int4(-1, 0, 0, 0);
+  if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(p.net.srow) + (size_t)k2 * 4 + lane);
+  spec.pw_k = -1;
+  if (__shfl_sync(0xffffffffu, ent.x, 0) == -2) return;     // more than 4 changed species: CSR walk
+  uint32_t lo = 0, hi = 0;
+  if (ent.x >= 0) { lo = (uint32_t)ent.z; hi = (uint32_t)ent.w; narrow_range(p.net, lo, hi, spec.k0, spec.k1); }
+  Ranges rg;
+  uint32_t acc = 0;
+#pragma unroll
+  for (int e = 0; e < 4; ++e) {
+    rg.lo[e] = __shfl_sync(0xffffffffu, lo, e);
+    acc += __shfl_sync(0xffffffffu, hi - lo, e);
+    rg.end[e] = acc;
+  }
+  uint32_t f = 0;
+  int n = 0;
+  if (!walk_scan(p.net, rg, f, spec.k0, spec.k1, lane, n, spec.pw_d, spec.pw_c)) {
+    spec.pw_k = k2; spec.pw_n = n; spec.pw_ent = ent;
+  }
 }
 
 
 // Fenced barrier over the CTAs of a bundle (start and end of a trajectory): all earlier global
 // writes of every CTA are visible to all later reads of every CTA.  Uses the exchange slots and
 // generation counter of bundle_argmin.  Returns false on a timeout.
-template <int BLOCK>
+template <int BLOCK, bool CLUSTER>
 __device__ __noinline__ bool bundle_barrier(u64 *exch, int S, int r, uint32_t gen, int *err) {
   __threadfence();
+  if (CLUSTER) {                                  // the bundle is one cluster: hardware barrier
+    cluster_barrier();
+    __threadfence();
+    return true;
+  }
   __syncthreads();
   bool ok = true;
   if (threadIdx.x < 32 && S > 1) {
@@ -656,10 +721,16 @@ __device__ __noinline__ bool bundle_barrier(u64 *exch, int S, int r, uint32_t ge
 // instantiation so that its code stays out of the instruction stream of the default kernel.
 // RATE = 1: a piecewise-constant rate schedule is set; RATE = 2: exponential rates c_k exp(lambda_k t)
 // (time-dependent rates, Eq.28): also their own instantiations.
-template <int BLOCK, bool SMEM, bool FULL, int RATE>
+// CLUSTER: the launch makes each bundle one thread-block cluster (S <= kMaxClusterCtas): the
+// exchange goes through distributed shared memory and `exch` is not used.
+template <int BLOCK, bool SMEM, bool FULL, int RATE, bool CLUSTER = false>
 __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams p) {
   constexpr bool SCHED = RATE == 1, EXPR = RATE == 2;
   constexpr int NT = BLOCK - 32 * kWalkerWarps;      // stream threads; the last warp walks
+  // FREE: the walker warp only ANNOUNCES its staged refreshes (bar.arrive) and runs ahead into the
+  // pre-walk of the likely next winner while the stream warps apply them, re-scan and reduce; the
+  // stream warps never wait for it except for the refreshes themselves.
+  constexpr bool FREE = SMEM && !FULL;
   __shared__ BundleCtx<BLOCK> ctx;
   __shared__ int list_k[kListCap];
   __shared__ int4 list_d[kListCap];
@@ -704,6 +775,11 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
   spec.sP = nullptr; spec.P_glob = nullptr; spec.k0 = 0; spec.seed = p.seed; spec.traj = 0;
   dirty[tid] = 0;
   if (tid == 0) { ctx.abort_local = 0; ctx.list_n = 0; ctx.more = 0; ctx.p_k = -1; ctx.any_odd = 0; }
+  if (CLUSTER && tid == 0) {     // (peers touch them only after the first bundle_barrier)
+    mbar_init(smem_addr(&ctx.cl_bar[0]), 1u);
+    mbar_init(smem_addr(&ctx.cl_bar[1]), 1u);
+    mbar_fence_init();
+  }
   __syncthreads();
   Cand none; none.dt = INF; none.k = 0x7fffffff;
 
@@ -716,8 +792,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     // ---- a-0: X = x0 (slices, version 0), then T = 0, P = E(k,0), a = a(X0), n = 0 for the own range
     for (int j = (r / p.G) * BLOCK + tid; j < N; j += ((p.S - xg + p.G - 1) / p.G) * BLOCK)
       __stcg(X + j, x_pack(0ull, p.x0[j]));
-    if (!bundle_barrier<BLOCK>(exch, p.S, r, gen, p.err)) return;
-    gen += 1u;
+    if (!bundle_barrier<BLOCK, CLUSTER>(exch, p.S, r, gen, p.err)) return;
+    if (!CLUSTER) gen += 1u;     // (a cluster's gen counts exchanges only: it is the mbarrier phase)
     for (int k = k0 + tid; k < (SMEM ? k0 + cnt_pad : k1); k += BLOCK) {
       double a0 = 0.0, p0 = 1.0;     // padding: a = 0, P - T = 1 > 0, so its q~ is +inf, never NaN
       double t_init = 0.0, p_init = 1.0;
@@ -917,6 +993,10 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           }
           if (pre_n < 0) walk_finish<SCHED>(p, fac, X, lane, n, list_d, list_k, list_a);
           if (lane == 0) { ctx.list_n = n; ctx.more = more ? 1 : 0; }
+          if (FREE && !more && !(SCHED && rate_change)) {      // run ahead (see FREE)
+            named_arrive<BLOCK>(kBarStaged);
+            break;
+          }
         } else if (first_round) {
           // ===== stream warps: a-5 of the previous firing fused with a-2/a-3 of this one =====
           bool defer = false;
@@ -925,7 +1005,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           mybest_k[tid] = defer ? -3 : best.k;
           if (defer) dirty[tid] = 1;
         }
-        __syncthreads();
+        if (FREE) named_sync<BLOCK>(kBarStaged); else __syncthreads();
         // ----- apply the staged refreshes; mark the owning threads for a re-scan
         const int n = ctx.list_n;
         const bool more = ctx.more != 0;
@@ -934,7 +1014,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
         // owner re-scans; otherwise the new waiting time simply joins the reduction as one more
         // candidate.  The reaction that fired (new P) always sends its owner to the re-scan.
         const int pk_now = ctx.p_k;
-        for (int i = tid; i < n; i += BLOCK) {
+        for (int i = tid; i < n && !(FREE && is_walker); i += (FREE ? NT : BLOCK)) {
           const int k = list_k[i];
           const double a_new = list_a[i];
           if (SMEM) sA[k - k0] = a_new; else __stcg(A + k, a_new);
@@ -956,7 +1036,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
           }
           ctx.n_stale = 0;
         }
-        __syncthreads();
+        if (FREE && !more && !(SCHED && rate_change)) named_sync<NT>(1);   // (the walker is not here)
+        else __syncthreads();
         if (!more) break;
         first_round = false;
       }
@@ -1034,7 +1115,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
       if (finishing) break;
 
       // ---- a-3 argmin over the bundle
-      const Cand win = bundle_argmin<BLOCK, SMEM>(p, ctx, exch, nfire, r, gen, best, spec);
+      const Cand win = bundle_argmin<BLOCK, SMEM, CLUSTER, FREE>(p, ctx, exch, nfire, r, gen, best, spec);
       if (win.k == -2) return;
 
       // ---- a-4 stop tests, identical in every thread of every CTA of the bundle
@@ -1077,8 +1158,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_bundle_kernel(const BundleParams 
     }
 
     // ---- trajectory done: every CTA's X updates are visible bundle-wide after the fenced barrier
-    if (!bundle_barrier<BLOCK>(exch, p.S, r, gen, p.err)) return;
-    gen += 1u;
+    if (!bundle_barrier<BLOCK, CLUSTER>(exch, p.S, r, gen, p.err)) return;
+    if (!CLUSTER) gen += 1u;
     dirty[tid] = 0;
     if (SMEM)
       for (int k = k0 + tid; k < k1; k += BLOCK) {

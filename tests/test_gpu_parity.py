@@ -58,11 +58,23 @@ def test_cfg3_scaled_trace(rt, scale, firings, refresh_mode):
                options=[("refresh_mode", refresh_mode)])
 
 
-@pytest.mark.parametrize("ctas", [1, 2, 7, 0])
-def test_cfg3_bundle_shape_invariance(rt, ctas):
-    """Result must not depend on how many CTAs share the trajectory (determinism contract)."""
+@pytest.mark.parametrize("exchange", [0, 1])
+@pytest.mark.parametrize("ctas", [1, 2, 7, 12, 16, 0])
+def test_cfg3_bundle_shape_invariance(rt, ctas, exchange):
+    """Result must not depend on how many CTAs share the trajectory (determinism contract), nor on
+    how they exchange their partial argmins: as one thread-block cluster through distributed
+    shared memory (exchange 0, bundles of 2..16 CTAs) or through slots in L2 (exchange 1)."""
     net, x0, par = W.make_config("cfg3", scale=0.02)
-    _check_run(rt, net, x0, par["seed"], 3, 1500, math.inf, 1500, options=[("bundle_ctas", ctas)])
+    _check_run(rt, net, x0, par["seed"], 3, 1500, math.inf, 1500,
+               options=[("bundle_ctas", ctas), ("exchange", exchange)])
+    with rt.Model(net) as m:
+        m.set_option("bundle_ctas", ctas)
+        m.set_option("exchange", exchange)
+        m.run(x0, par["seed"], 3, 10)
+        S = m.info("bundle_ctas")
+        assert m.info("cluster_exchange") == (1 if exchange == 0 and 2 <= S <= 16 else 0)
+        if ctas:
+            assert S == ctas
 
 
 @pytest.mark.parametrize("state_mode", [0, 1])
@@ -96,13 +108,13 @@ def _hub_network(n_species=40, n_reactions=5000, seed=3):
     return W.from_reactions(n_species, reactions), rng.integers(20, 60, size=n_species).astype(np.int64)
 
 
-@pytest.mark.parametrize("ctas,state_mode", [(1, 0), (1, 1), (5, 0), (0, 0)])
-def test_hub_species_general_rows_and_staging_overflow(rt, ctas, state_mode):
+@pytest.mark.parametrize("ctas,state_mode,exchange", [(1, 0, 0), (1, 1, 0), (5, 0, 0), (5, 0, 1), (0, 0, 0), (0, 0, 1)])
+def test_hub_species_general_rows_and_staging_overflow(rt, ctas, state_mode, exchange):
     net, x0 = _hub_network()
     for refresh_mode in (0, 1):
         _check_run(rt, net, x0, 21, 0, 600, math.inf, 600,
                    options=[("bundle_ctas", ctas), ("state_mode", state_mode),
-                            ("refresh_mode", refresh_mode)])
+                            ("refresh_mode", refresh_mode), ("exchange", exchange)])
 
 
 @pytest.mark.parametrize("ctas", [1, 0])
@@ -207,14 +219,15 @@ def _check_tie(rt, M, coupled, formulation, options, n_more=40):
 
 
 @pytest.mark.parametrize("formulation", [0, 1])
-@pytest.mark.parametrize("state_mode", [0, 1])
-@pytest.mark.parametrize("ctas", [1, 3, 7, 0])
+@pytest.mark.parametrize("state_mode", [0, 1, 2])
+@pytest.mark.parametrize("ctas", [1, 3, 7, 16, 0])
 def test_exact_ties_go_to_the_lowest_index(rt, ctas, state_mode, formulation):
     """north_star: "argmin reduction over k with ties broken by lowest index".  The ties straddle
     the reactions of one thread (filter fallback: every approximate quotient of a thread is equal),
     lanes, warps and CTAs (REDUX lexmin, exchange slots), and with `coupled` every firing refreshes
     every hub reader inside the tie (fresh-candidate merge, warp-shared / cooperative re-scan)."""
-    opts = [("bundle_ctas", ctas), ("state_mode", state_mode)]
+    # state_mode 2 here: state in shared memory with the exchange through L2 (0: cluster / DSMEM)
+    opts = [("bundle_ctas", ctas), ("state_mode", state_mode & 1), ("exchange", 1 if state_mode == 2 else 0)]
     _check_tie(rt, 5003, False, formulation, opts)
     _check_tie(rt, 4999, True, formulation, opts)
 
@@ -290,7 +303,8 @@ def test_resume_argument_checks(rt):
 def test_cfg3_full_first_1e4(rt):
     """BASELINE config 3 at full size: first 1e4 firings bit-exact."""
     net, x0, par = W.make_config("cfg3")
-    _check_run(rt, net, x0, par["seed"], 0, 10_000, math.inf, 10_000)
+    _check_run(rt, net, x0, par["seed"], 0, 10_000, math.inf, 10_000)     # one 16-CTA cluster
+    _check_run(rt, net, x0, par["seed"], 0, 10_000, math.inf, 10_000, options=[("exchange", 1)])   # 148 CTAs, L2
 
 
 def test_cfg4_scaled(rt):
