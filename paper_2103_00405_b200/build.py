@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librt_b200.so")
 SOURCES = ["rt_api.cu"]
-HEADERS = ["rt_device.cuh", "rt_bundle.cuh", "rt_thread.cuh", os.path.join("..", "..", "include", "rt.h")]
+HEADERS = ["rt_device.cuh", "rt_bundle.cuh", "rt_fast.cuh", "rt_thread.cuh", os.path.join("..", "..", "include", "rt.h")]
 
 
 def _stale():

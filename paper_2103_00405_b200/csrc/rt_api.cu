@@ -14,6 +14,7 @@
 
 #include "../../include/rt.h"
 #include "rt_bundle.cuh"
+#include "rt_fast.cuh"
 #include "rt_thread.cuh"
 
 using rt::u64;
@@ -24,6 +25,9 @@ using rt::u64;
 #ifndef RT_BLOCK_GLOBAL
 #define RT_BLOCK_GLOBAL 512
 #endif
+#ifndef RT_BLOCK_FAST
+#define RT_BLOCK_FAST 256
+#endif
 namespace {
 
 // Threads per CTA of the bundle kernel (stream warps + 1 walker warp).  Measured on B200: with
@@ -33,6 +37,8 @@ namespace {
 // 55.7 us, 384: 58.2, 256: 65.4).
 constexpr int kBlockSmem = RT_BLOCK_SMEM;
 constexpr int kBlockGlobal = RT_BLOCK_GLOBAL;
+constexpr int kBlockFast = RT_BLOCK_FAST;                      // candidate-first kernel (rt_fast.cuh)
+constexpr size_t kSmemStateBytesFast = 206 * 1024;             // (its static shared memory is larger)
 constexpr int kThreadKernelMaxM = 64; // one-thread-per-trajectory path: M, N at most this
 constexpr int kMinPairsPerCta = 256;  // do not spread a trajectory thinner than this
 constexpr int kBigDeg = 64;           // species read by more reactions than this get a block-offset table
@@ -87,7 +93,8 @@ struct rt_model {
   DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t, d_T0, d_P0, d_n0;
   // options
   int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0, opt_prefetch = 7, opt_formulation = 0;
-  int opt_exchange = 0;
+  int opt_exchange = 0, opt_pipeline = 1;
+  int last_fast = 0;
   int max_clusters[rt::kMaxClusterCtas + 1] = {};   // co-resident clusters per cluster size (0 = not asked yet, -1 = none)
   int last_cluster = 0;
   // info
@@ -163,18 +170,27 @@ struct StartDev {
 
 // How one launch is shaped: B bundles of S CTAs; smem = the (T,P,a) state lives in shared memory.
 // cluster = each bundle is one thread-block cluster and exchanges through distributed shared memory.
-struct Plan { int S, B, G; int pairs_per_cta; int cnt_pad; bool smem; bool cluster; };
+// fast = the candidate-first kernel of rt_fast.cuh (on-chip state, dependency refresh, constant rates).
+struct Plan { int S, B, G; int pairs_per_cta; int cnt_pad; bool smem; bool cluster; bool fast; };
 
+// stream threads of the kernel that keeps the state in shared memory
+int stream_threads(bool fast) {
+  return fast ? kBlockFast - 32 * rt::kFastHelperWarps : kBlockSmem - 32 * rt::kWalkerWarps;
+}
+size_t smem_budget(bool fast) { return fast ? kSmemStateBytesFast : kSmemStateBytes; }
 // slots per shared-memory state array: a CTA's reactions padded to whole scan batches
-int padded_count(int pairs_per_cta) {
-  const int batch = rt::kScanBatch * (kBlockSmem - 32 * rt::kWalkerWarps);
+int padded_count(int pairs_per_cta, bool fast) {
+  const int batch = rt::kScanBatch * stream_threads(fast);
   return (2 * pairs_per_cta + batch - 1) / batch * batch;
 }
-size_t smem_state_bytes(int pairs_per_cta) { return (size_t)padded_count(pairs_per_cta) * 3 * sizeof(double); }
+size_t smem_state_bytes(int pairs_per_cta, bool fast) {
+  return (size_t)padded_count(pairs_per_cta, fast) * 3 * sizeof(double);
+}
 
 // The bundle kernel for a launch shape (FULL = refresh_mode 1; rate: 0 constant, 1 schedule, 2 exponential).
-const void *bundle_kernel(bool smem, bool full, int rate, bool cluster) {
+const void *bundle_kernel(bool smem, bool full, int rate, bool cluster, bool fast = false) {
   using namespace rt;
+  if (fast) return cluster ? (const void *)rt_fast_kernel<kBlockFast, true> : (const void *)rt_fast_kernel<kBlockFast, false>;
   if (smem && cluster)
     return full        ? (const void *)rt_bundle_kernel<kBlockSmem, true, true, 0, true>
            : rate == 1 ? (const void *)rt_bundle_kernel<kBlockSmem, true, false, 1, true>
@@ -196,8 +212,8 @@ const void *bundle_kernel(bool smem, bool full, int rate, bool cluster) {
 int max_active_clusters(rt_model *m, int S) {
   if (S < 2 || S > rt::kMaxClusterCtas) return 0;
   if (m->max_clusters[S] == 0) {
-    const void *kern = bundle_kernel(true, false, 0, true);
-    int n = 0;
+    const void *kern = bundle_kernel(true, false, 0, true);     // (the same count holds for rt_fast_kernel:
+    int n = 0;                                                   //  one CTA per SM either way)
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(S); cfg.blockDim = dim3(kBlockSmem); cfg.dynamicSmemBytes = kSmemStateBytes;
     cudaLaunchAttribute at[1];
@@ -215,12 +231,25 @@ int max_active_clusters(rt_model *m, int S) {
   return std::max(m->max_clusters[S], 0);
 }
 
+Plan plan_bundles_for(rt_model *m, u64 n_traj, bool fast);
+
 Plan plan_bundles(rt_model *m, u64 n_traj) {
+  // the candidate-first kernel covers the default configuration: on-chip state, dependency refresh,
+  // constant rates, one copy of X
+  const bool fast = m->opt_pipeline != 0 && m->refresh_mode == 0 && m->sched_n == 0 && !m->rate_exp &&
+                    m->opt_x_replicas <= 1 && m->opt_state_mode != 1;
+  Plan pl = plan_bundles_for(m, n_traj, fast);
+  // (its static shared memory is larger: at the capacity edge only the plain kernel still fits)
+  if (fast && !pl.smem) pl = plan_bundles_for(m, n_traj, false);
+  return pl;
+}
+
+Plan plan_bundles_for(rt_model *m, u64 n_traj, bool fast) {
   const int pairs_total = m->net.M_pad / 2;
   const int sms = m->num_sms;
   // fewest CTAs whose share of the state still fits in shared memory
-  const int batch = rt::kScanBatch * (kBlockSmem - 32 * rt::kWalkerWarps);
-  const int pairs_fit = std::max(1, (int)(kSmemStateBytes / (3 * sizeof(double)) / batch * batch / 2));
+  const int batch = rt::kScanBatch * stream_threads(fast);
+  const int pairs_fit = std::max(1, (int)(smem_budget(fast) / (3 * sizeof(double)) / batch * batch / 2));
   const int s_fit = (pairs_total + pairs_fit - 1) / pairs_fit;
   const int s_thin = std::max(1, (pairs_total + kMinPairsPerCta - 1) / kMinPairsPerCta);
   const bool may_cluster = m->opt_exchange != 1 && m->opt_state_mode != 1;
@@ -256,8 +285,9 @@ Plan plan_bundles(rt_model *m, u64 n_traj) {
   Plan pl;
   pl.S = S;
   pl.pairs_per_cta = (pairs_total + S - 1) / S;
-  pl.cnt_pad = padded_count(pl.pairs_per_cta);
-  pl.smem = m->opt_state_mode != 1 && smem_state_bytes(pl.pairs_per_cta) <= kSmemStateBytes;
+  pl.smem = m->opt_state_mode != 1 && smem_state_bytes(pl.pairs_per_cta, fast) <= smem_budget(fast);
+  pl.fast = fast && pl.smem;
+  pl.cnt_pad = padded_count(pl.pairs_per_cta, pl.fast);
   if (may_cluster && pl.smem && S >= 2 && S <= rt::kMaxClusterCtas) {
     B = (int)std::min<u64>(std::max<u64>(n_traj, 1), (u64)max_active_clusters(m, S));
     cluster = B >= 1;
@@ -315,10 +345,10 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.err = (int *)m->d_err.p;
   void *args[] = {&p};
   const int rate = m->sched_n > 0 ? 1 : m->rate_exp ? 2 : 0;   // (never with refresh_mode 1: checked above)
-  const void *kern = bundle_kernel(pl.smem, m->refresh_mode != 0, rate, pl.cluster);
-  const size_t dyn = pl.smem ? smem_state_bytes(pl.pairs_per_cta) : 0;
+  const void *kern = bundle_kernel(pl.smem, m->refresh_mode != 0, rate, pl.cluster, pl.fast);
+  const size_t dyn = pl.smem ? smem_state_bytes(pl.pairs_per_cta, pl.fast) : 0;
   if (dyn) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-  const int block = pl.smem ? kBlockSmem : kBlockGlobal;
+  const int block = pl.fast ? kBlockFast : pl.smem ? kBlockSmem : kBlockGlobal;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(pl.S * pl.B); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = dyn; cfg.stream = st;
   cudaLaunchAttribute at[1];
@@ -339,6 +369,7 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   m->kernel_launches += 1;
   m->last_S = pl.S; m->last_B = pl.B; m->last_path = 2; m->last_state_smem = pl.smem ? 1 : 0;
   m->last_cluster = pl.cluster ? 1 : 0;
+  m->last_fast = pl.fast ? 1 : 0;
   return RT_OK;
 }
 
@@ -757,6 +788,9 @@ int rt_set_option(rt_model *m, const char *name, int64_t value) {
   } else if (!strcmp(name, "state_mode")) {
     if (value < 0 || value > 1) return RT_ERR_BAD_ARG;
     m->opt_state_mode = (int)value;
+  } else if (!strcmp(name, "pipeline")) {
+    if (value < 0 || value > 1) return RT_ERR_BAD_ARG;
+    m->opt_pipeline = (int)value;
   } else if (!strcmp(name, "exchange")) {
     if (value < 0 || value > 1) return RT_ERR_BAD_ARG;
     m->opt_exchange = (int)value;
@@ -778,6 +812,7 @@ int rt_get_info(const rt_model *m, const char *name, int64_t *value) {
   else if (!strcmp(name, "max_sigma")) *value = m->max_sigma;
   else if (!strcmp(name, "state_in_smem")) *value = m->last_state_smem;
   else if (!strcmp(name, "cluster_exchange")) *value = m->last_cluster;
+  else if (!strcmp(name, "pipeline")) *value = m->last_fast;
   else if (!strcmp(name, "hub_species")) *value = (int64_t)m->n_big;
   else return RT_ERR_BAD_ARG;
   return RT_OK;

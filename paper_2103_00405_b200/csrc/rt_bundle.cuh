@@ -500,9 +500,83 @@ struct Spec {
   double *pw_c;
 };
 
-// Block-wide lexmin of the thread candidates, then all-gather of the S CTA partials through the
-// exchange slots (which is also the per-firing bundle barrier).  Every thread returns the
-// bundle-wide winner.  win.k == -2 signals a timeout.
+// All-gather of the S CTA partials of a bundle (one warp; every lane holds this CTA's partial in
+// `c`): through distributed shared memory when the bundle is one cluster, else through the exchange
+// slots in L2.  Doubles as the per-firing bundle barrier.  On return every lane holds the
+// bundle-wide winner in `c` (c.k == -2: timeout) and the runner-up in `c2`.
+// `between` runs after this CTA has posted and before it waits (work hidden behind the exchange).
+struct NoWork { __device__ __forceinline__ void operator()() const {} };
+template <bool CLUSTER, typename Between = NoWork>
+__device__ __forceinline__ void exchange_partials(const BundleParams &p, u64 (*cl_slot)[kMaxClusterCtas][2],
+                                                  u64 *cl_bar, u64 *exch, int r, uint32_t gen, int lane,
+                                                  Cand &c, Cand &c2, Between between = Between()) {
+  c2.dt = __longlong_as_double(0x7ff0000000000000ll); c2.k = 0x7fffffff;
+  if (CLUSTER && p.S > 1) {
+    // One thread-block cluster = one bundle: lane l stores this CTA's partial into slot r of
+    // peer l (st.async: the store also completes 16 bytes on the peer's mbarrier), then every
+    // CTA waits for its own 16 * S bytes.  No global memory on the path.
+    const uint32_t par = gen & 1u, ph = (gen >> 1) & 1u;
+    const uint32_t bar = smem_addr(&cl_bar[par]);
+    if (lane == 0) mbar_arrive_expect_tx(bar, 16u * (uint32_t)p.S);
+    if (lane < p.S)
+      st_async_v2(mapa_u32(smem_addr(&cl_slot[par][r][0]), (uint32_t)lane),
+                  (u64)__double_as_longlong(c.dt), (u64)(uint32_t)c.k, mapa_u32(bar, (uint32_t)lane));
+    between();
+    const long long t0 = clock64();
+    bool timed_out = false;
+    while (!mbar_try_wait(bar, ph))
+      if (clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); timed_out = true; break; }
+    Cand s;
+    s.dt = __longlong_as_double(0x7ff0000000000000ll); s.k = 0x7fffffff;
+    if (lane < p.S) {
+      s.dt = __longlong_as_double((long long)cl_slot[par][lane][0]);
+      s.k = (int)(uint32_t)cl_slot[par][lane][1];
+    }
+    c = warp_lexmin(s);
+    if (s.k == c.k) { s.dt = __longlong_as_double(0x7ff0000000000000ll); s.k = 0x7fffffff; }
+    c2 = warp_lexmin(s);                        // runner-up: best of everything but the winner
+    if (__any_sync(0xffffffffu, timed_out)) c.k = -2;
+  } else if (p.S > 1) {
+    const uint32_t tag = gen + 1u;
+    const u64 par = (u64)(((gen >> 1) & 1u) ^ 1u) << 63;     // never matches zeroed memory
+    u64 *buf = exch + (size_t)(gen & 1u) * (size_t)p.S * kSlotStride;
+    if (lane == 0)
+      st_relaxed_v2(buf + (size_t)kSlotStride * r, (u64)__double_as_longlong(c.dt) | par,
+                    ((u64)tag << 32) | (u64)(uint32_t)c.k);
+    between();
+    c.dt = __longlong_as_double(0x7ff0000000000000ll);
+    c.k = 0x7fffffff;
+    const long long t0 = clock64();
+    // Lane l gathers slots l, l+32, ...: all of its loads are in flight together, so the
+    // all-gather completes one L2 round trip after the last CTA has posted.
+    constexpr int kMaxPer = kMaxBundleCtas / 32;
+    unsigned pending = 0;
+    for (int i = 0; i < kMaxPer; ++i) if (lane + 32 * i < p.S) pending |= 1u << i;
+    while (pending) {
+      u64 w0[kMaxPer], w1[kMaxPer];
+#pragma unroll
+      for (int i = 0; i < kMaxPer; ++i)
+        if (pending & (1u << i)) ld_relaxed_v2(buf + (size_t)kSlotStride * (lane + 32 * i), w0[i], w1[i]);
+#pragma unroll
+      for (int i = 0; i < kMaxPer; ++i)
+        if ((pending & (1u << i)) && (uint32_t)(w1[i] >> 32) == tag && (w0[i] >> 63) == (par >> 63)) {
+          pending &= ~(1u << i);
+          const double dt = __longlong_as_double((long long)(w0[i] & 0x7fffffffffffffffull));
+          const int k = (int)(uint32_t)(w1[i] & 0x7fffffffu);
+          if (cand_less(dt, k, c)) { c2 = c; c.dt = dt; c.k = k; }
+          else if (cand_less(dt, k, c2)) { c2.dt = dt; c2.k = k; }
+        }
+      if (pending && clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); c.k = -2; break; }
+    }
+    const bool timed_out = __any_sync(0xffffffffu, c.k == -2);
+    const Cand mine_best = c;
+    c = warp_lexmin(c);
+    // runner-up = best of everything but the winner: the likeliest winner of the next firing
+    c2 = warp_lexmin((mine_best.k == c.k) ? c2 : mine_best);
+    if (timed_out) c.k = -2;
+  }
+}
+
 // Named barriers of the kernel: 0 = __syncthreads; 1 = the stream warps among themselves; 2 = warp 0
 // hands the winner to the walker warp; 3 = the walker's staged refreshes are ready (kBarStaged);
 // 4 = the stream warps' partials are ready for the walker (kBarParts).
@@ -519,6 +593,9 @@ template <int COUNT> __device__ __forceinline__ void named_arrive(int id) {
 // pw_d / pw_c.  Network data only, so it stays valid until another reaction is pre-walked.
 __device__ __forceinline__ void prewalk(const BundleParams &p, Spec &spec, int lane);
 
+// Block-wide lexmin of the thread candidates, then all-gather of the S CTA partials (exchange_partials,
+// which is also the per-firing bundle barrier).  Every thread returns the
+// bundle-wide winner.  win.k == -2 signals a timeout.
 // FREE: the walker warp runs ahead of the stream warps (see the kernel): it does not post a partial
 // and pre-walks BEFORE it waits for the stream warps' partials.
 template <int BLOCK, bool PREWALK, bool CLUSTER, bool FREE>
@@ -549,68 +626,7 @@ __device__ __forceinline__ Cand bundle_argmin(const BundleParams &p, BundleCtx<B
     c = warp_lexmin(c);
     Cand c2;                                      // this lane's second-best slot (runner-up search)
     c2.dt = __longlong_as_double(0x7ff0000000000000ll); c2.k = 0x7fffffff;
-    if (CLUSTER && p.S > 1) {
-      // One thread-block cluster = one bundle: lane l stores this CTA's partial into slot r of
-      // peer l (st.async: the store also completes 16 bytes on the peer's mbarrier), then every
-      // CTA waits for its own 16 * S bytes.  No global memory on the path.
-      const uint32_t par = gen & 1u, ph = (gen >> 1) & 1u;
-      const uint32_t bar = smem_addr(&ctx.cl_bar[par]);
-      if (lane == 0) mbar_arrive_expect_tx(bar, 16u * (uint32_t)p.S);
-      if (lane < p.S)
-        st_async_v2(mapa_u32(smem_addr(&ctx.cl_slot[par][r][0]), (uint32_t)lane),
-                    (u64)__double_as_longlong(c.dt), (u64)(uint32_t)c.k, mapa_u32(bar, (uint32_t)lane));
-      const long long t0 = clock64();
-      bool timed_out = false;
-      while (!mbar_try_wait(bar, ph))
-        if (clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); timed_out = true; break; }
-      Cand s;
-      s.dt = __longlong_as_double(0x7ff0000000000000ll); s.k = 0x7fffffff;
-      if (lane < p.S) {
-        s.dt = __longlong_as_double((long long)ctx.cl_slot[par][lane][0]);
-        s.k = (int)(uint32_t)ctx.cl_slot[par][lane][1];
-      }
-      c = warp_lexmin(s);
-      if (s.k == c.k) { s.dt = __longlong_as_double(0x7ff0000000000000ll); s.k = 0x7fffffff; }
-      c2 = warp_lexmin(s);                        // runner-up: best of everything but the winner
-      if (__any_sync(0xffffffffu, timed_out)) c.k = -2;
-    } else if (p.S > 1) {
-      const uint32_t tag = gen + 1u;
-      const u64 par = (u64)(((gen >> 1) & 1u) ^ 1u) << 63;     // never matches zeroed memory
-      u64 *buf = exch + (size_t)(gen & 1u) * (size_t)p.S * kSlotStride;
-      if (lane == 0)
-        st_relaxed_v2(buf + (size_t)kSlotStride * r, (u64)__double_as_longlong(c.dt) | par,
-                      ((u64)tag << 32) | (u64)(uint32_t)c.k);
-      c.dt = __longlong_as_double(0x7ff0000000000000ll);
-      c.k = 0x7fffffff;
-      const long long t0 = clock64();
-      // Lane l gathers slots l, l+32, ...: all of its loads are in flight together, so the
-      // all-gather completes one L2 round trip after the last CTA has posted.
-      constexpr int kMaxPer = kMaxBundleCtas / 32;
-      unsigned pending = 0;
-      for (int i = 0; i < kMaxPer; ++i) if (lane + 32 * i < p.S) pending |= 1u << i;
-      while (pending) {
-        u64 w0[kMaxPer], w1[kMaxPer];
-#pragma unroll
-        for (int i = 0; i < kMaxPer; ++i)
-          if (pending & (1u << i)) ld_relaxed_v2(buf + (size_t)kSlotStride * (lane + 32 * i), w0[i], w1[i]);
-#pragma unroll
-        for (int i = 0; i < kMaxPer; ++i)
-          if ((pending & (1u << i)) && (uint32_t)(w1[i] >> 32) == tag && (w0[i] >> 63) == (par >> 63)) {
-            pending &= ~(1u << i);
-            const double dt = __longlong_as_double((long long)(w0[i] & 0x7fffffffffffffffull));
-            const int k = (int)(uint32_t)(w1[i] & 0x7fffffffu);
-            if (cand_less(dt, k, c)) { c2 = c; c.dt = dt; c.k = k; }
-            else if (cand_less(dt, k, c2)) { c2.dt = dt; c2.k = k; }
-          }
-        if (pending && clock64() - t0 > kSpinLimitCycles) { atomicExch(p.err, 1); c.k = -2; break; }
-      }
-      const bool timed_out = __any_sync(0xffffffffu, c.k == -2);
-      const Cand mine_best = c;
-      c = warp_lexmin(c);
-      // runner-up = best of everything but the winner: the likeliest winner of the next firing
-      c2 = warp_lexmin((mine_best.k == c.k) ? c2 : mine_best);
-      if (timed_out) c.k = -2;
-    }
+    exchange_partials<CLUSTER>(p, ctx.cl_slot, ctx.cl_bar, exch, r, gen, lane, c, c2);
     if (lane == 0) { ctx.win = c; ctx.second_k = (c2.dt < __longlong_as_double(0x7ff0000000000000ll)) ? c2.k : 0x7fffffff; }
   } else if (walker) {
     // Walker warp, idle during the exchange.  If this CTA's candidate wins (it usually stays the

@@ -1,0 +1,584 @@
+// rt_fast.cuh -- "candidate-first" bundle kernel: the per-firing O(M) pass is taken OFF the critical
+// path of a firing.  Same algorithm, same arithmetic, same results as rt_bundle_kernel (state in
+// shared memory, dependency-graph refresh, constant rates, either formulation); what changes is
+// WHEN each piece of a firing's work is done.
+//
+// In rt_bundle_kernel one firing is  pass over all reactions -> block argmin -> exchange, so the
+// exchange (1.2 us through L2, 0.27 us inside a cluster) and the pass (1.3 us) add up.  Here every
+// stream thread carries ONE candidate, the reaction the previous pass found to be the thread's
+// argmin with a safety margin (below).  After an exchange has named (mu, dt):
+//   S1  each thread advances only its candidate, T_c += a_c dt, and divides it exactly;
+//   S2  the reactions whose propensity changed (the walker's staged list) are advanced with their
+//       OLD a_k, get the new a_k, and join the reduction as fresh candidates;
+//   S3  threads whose candidate fired or was refreshed (or that have none) are re-scanned exactly,
+//       their warp sharing the work;
+//   S4  block argmin -> the exchange warp posts this CTA's partial;
+//   S5  WHILE the exchange is in flight the stream warps run the pass: T_k += a_k dt for every
+//       reaction not advanced in S1..S3 (per-thread bit masks), approximate quotients, and the
+//       choice of the thread's candidate for the NEXT firing.
+// Every T_k still receives every increment a_k dt_n, one rounded multiply and one rounded add per
+// firing, in firing order: results are bit-identical to dividing everything every firing.
+//
+// Why a candidate chosen one firing early is still the thread's exact argmin:
+// the pass looks at the HIGH WORD of q~_k = (P_k - T_k) * rcp.approx(a_k) as an integer key
+// (positive doubles order like integers).  Key error: rcp.approx.ftz.f64 2^-19.9 relative
+// (tests/test_gpu_kernel_facts.py), truncation < 1 unit; a unit is 2^-20..2^-21 relative, so a key
+// is within 3.5 units of the exact quotient's.  One more firing moves every exact quotient of the
+// thread by the same dt, except for the rounding of T_k + a_k dt, which is at most
+// 2^-51 max(|T_k|, |P_k|) / a_k: the pass checks that P_k - T_k keeps at least 2^-31 of
+// max(|P_k|, |T_k|) (kGuardShift; integer test on high words), which bounds that error by 2 units.
+// A thread whose second-smallest key exceeds the smallest by more than kQTolUnits = 32 > 2 (3.5 + 2)
+// therefore has a unique exact argmin after the next firing too; any other thread has no candidate
+// and is re-scanned exactly (S3), as are all threads when some a_k of the CTA is outside the range
+// where the rcp bound is established (any_odd).
+//
+// Warps: NT / 32 stream warps, one exchange warp (reduces the warp partials, posts, precomputes the
+// redraw of this CTA's candidate while the exchange is in flight, gathers), one walker warp (X
+// update, staged refreshes; while the others work it pre-walks the exchange's runner-up AND
+// computes that reaction's refreshes speculatively from X as it will be, so that a correct guess
+// -- 94..99 % of the firings -- costs no memory round trip at all).
+#pragma once
+#include "rt_bundle.cuh"
+
+namespace rt {
+
+constexpr int kFastHelperWarps = 2;
+constexpr int kBarMore = 5, kBarWin = 6;
+constexpr int kQTolUnits = 32;       // key margin, in units of the high word's last bit
+constexpr int kGuardShift = 29;      // high word of P - T may be at most this many binades below max(|P|, |T|)'s
+
+template <int BLOCK>
+struct FastCtx {
+  Cand warp_part[(BLOCK - 32 * kFastHelperWarps) / 32];
+  Cand win;
+  int second_k;
+  int abort_local, list_n, list_buf, more, any_odd;
+  int p_k;                // reaction whose P was redrawn (or -1), and its new value
+  double p_val;
+  int spec_k;             // exchange warp -> walker: precomputed redraw of this CTA's candidate
+  uint32_t spec_n;
+  double spec_P;
+  alignas(16) u64 cl_slot[2][kMaxClusterCtas][2];
+  alignas(8) u64 cl_bar[2];
+};
+
+// Integer key of the approximate quotient of one reaction; clears guard_ok when the lagged
+// candidate argument does not cover it (see the header).
+__device__ __forceinline__ int q_key(double pk, double t, double a, bool &guard_ok) {
+  const double r = __dsub_rn(pk, t);
+  const int hq = __double2hiint(__dmul_rn(r, rcp_approx(a)));
+  const int hm = max(__double2hiint(pk) & 0x7fffffff, __double2hiint(t) & 0x7fffffff);
+  guard_ok = guard_ok && ((__double2hiint(r) + (kGuardShift << 20) >= hm) || hq >= 0x7ff00000);
+  return hq;
+}
+
+// S5: the pass of one thread.  Advances the reactions whose bit in `done` is clear, then picks the
+// candidate slot for the next firing (-1: none, the thread will be re-scanned exactly).
+template <int NT>
+__device__ __forceinline__ int pass_and_pick(int tid, int cnt_pad, double *__restrict__ sT,
+                                             const double *__restrict__ sP, const double *__restrict__ sA,
+                                             double dprev, u64 done, bool any_odd) {
+  constexpr int U = kScanBatch;
+  int m1 = 0x7fffffff, m2 = 0x7fffffff, s1 = 0;
+  bool guard_ok = true;
+  int slot = 0;
+  for (int i = tid; i < cnt_pad; i += U * NT, slot += U) {
+    double a[U], t[U], pk[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) { a[u] = sA[i + u * NT]; t[u] = sT[i + u * NT]; pk[u] = sP[i + u * NT]; }
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+      if (!((done >> (slot + u)) & 1ull)) {
+        t[u] = __dadd_rn(t[u], __dmul_rn(a[u], dprev));
+        sT[i + u * NT] = t[u];
+      }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int q = q_key(pk[u], t[u], a[u], guard_ok);
+      m2 = min(m2, max(q, m1));
+      if (q < m1) { m1 = q; s1 = slot + u; }
+    }
+  }
+  const bool decided = !any_odd && guard_ok && m1 >= ((1023 - 100) << 20) && m1 <= ((1023 + 100) << 20) &&
+                       m2 > m1 + kQTolUnits;
+  return decided ? s1 : -1;
+}
+
+template <int BLOCK, bool CLUSTER>
+__global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p) {
+  constexpr int NT = BLOCK - 32 * kFastHelperWarps;   // stream threads
+  constexpr int XW = NT / 32;                         // exchange warp
+  constexpr int WW = NT / 32 + 1;                     // walker warp
+  __shared__ FastCtx<BLOCK> ctx;
+  __shared__ int out_k[2][kListCap];                  // staged refreshes (k, new a_k), two buffers:
+  __shared__ double out_a[2][kListCap];               //   one published, one being speculated into
+  __shared__ int4 list_d[kListCap];
+  __shared__ int4 pw_d[kListCap];                     // pre-walked dependency entries of reaction pw_k
+  __shared__ double pw_c[kListCap];
+  __shared__ u64 advm[NT];                            // per stream thread: slots already advanced this firing
+  __shared__ u64 refm[NT];                            //                    slots whose refresh is claimed
+  __shared__ int mybest_k[NT];                        // reaction each stream thread proposes (-3: none)
+  __shared__ unsigned char dirty[NT];
+  extern __shared__ __align__(16) unsigned char dyn_smem[];
+  const NetDev &net = p.net;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const bool is_stream = warp < XW, is_xw = warp == XW, is_walker = warp == WW;
+  const int b = blockIdx.x / p.S, r = blockIdx.x % p.S;
+  const int M = net.M, N = net.N;
+  const double INF = __longlong_as_double(0x7ff0000000000000ll);
+  const bool resid = p.formulation != 0;
+
+  double *T = p.T + (size_t)b * net.M_pad;
+  double *P = p.P + (size_t)b * net.M_pad;
+  double *A = p.a + (size_t)b * net.M_pad;
+  uint32_t *nfire = p.n + (size_t)b * net.M_pad;
+  u64 *X = p.X + (size_t)b * (size_t)N;
+  u64 *exch = p.exch + (size_t)b * 2 * p.S * kSlotStride;
+
+  const int pairs_total = net.M_pad / 2;
+  const int q0 = min(r * p.pairs_per_cta, pairs_total);
+  const int q1 = min(q0 + p.pairs_per_cta, pairs_total);
+  const int k0 = 2 * q0, k1 = 2 * q1;
+  const int cnt_pad = p.cnt_pad;
+  const int nslot = cnt_pad / NT;                     // slots per stream thread (<= 64)
+  double *sT = reinterpret_cast<double *>(dyn_smem);
+  double *sP = sT + cnt_pad;
+  double *sA = sP + cnt_pad;
+
+  uint32_t gen = 0;
+  if (tid == 0) {
+    ctx.abort_local = 0; ctx.list_n = 0; ctx.list_buf = 0; ctx.more = 0; ctx.p_k = -1; ctx.any_odd = 0;
+    ctx.spec_k = -1; ctx.second_k = 0x7fffffff;
+  }
+  if (CLUSTER && tid == 0) {
+    mbar_init(smem_addr(&ctx.cl_bar[0]), 1u);
+    mbar_init(smem_addr(&ctx.cl_bar[1]), 1u);
+    mbar_fence_init();
+  }
+  if (is_stream) { dirty[tid] = 0; advm[tid] = 0; refm[tid] = 0; mybest_k[tid] = -3; }
+  __syncthreads();
+  Cand none; none.dt = INF; none.k = 0x7fffffff;
+
+  for (u64 it = (u64)b; it < p.n_traj; it += (u64)p.B) {
+    const u64 traj = p.traj_first + it;
+    const bool tracing = (it == 0) && p.trace_cap > 0 && r == 0;
+
+    // ---- a-0: X = x0 (version 0), then T = 0, P = E(k,0), a = a(X0), n = 0 for the own range
+    for (int j = r * BLOCK + tid; j < N; j += p.S * BLOCK) __stcg(X + j, x_pack(0ull, p.x0[j]));
+    if (!bundle_barrier<BLOCK, CLUSTER>(exch, p.S, r, gen, p.err)) return;
+    if (!CLUSTER) gen += 1u;
+    for (int k = k0 + tid; k < k0 + cnt_pad; k += BLOCK) {
+      double a0 = 0.0, t_init = 0.0, p_init = 1.0;   // padding: a = 0, P - T = 1: key +inf, never NaN
+      uint32_t n_init = 0u;
+      if (k < k1 && k < M) {
+        a0 = propensity(net, X, k);
+        if (filter_unsafe(a0)) ctx.any_odd = 1;
+        if (p.T0) {
+          t_init = __ldg(p.T0 + k); p_init = __ldg(p.P0 + k); n_init = __ldg(p.n0 + k);
+        } else {
+          const double e0 = exp_draw(p.seed, traj, (uint32_t)k, 0u);
+          t_init = resid ? -e0 : 0.0; p_init = resid ? 0.0 : e0;
+        }
+      } else if (resid) { t_init = -1.0; p_init = 0.0; }
+      sT[k - k0] = t_init; sP[k - k0] = p_init; sA[k - k0] = a0;
+      if (k < k1) nfire[k] = n_init;
+    }
+    __syncthreads();
+    // candidates of the first firing (nothing to advance)
+    int cand_slot = -1;
+    if (is_stream) {
+      cand_slot = pass_and_pick<NT>(tid, cnt_pad, sT, sP, sA, 0.0, ~0ull, ctx.any_odd != 0);
+      mybest_k[tid] = cand_slot >= 0 ? k0 + tid + cand_slot * NT : -3;
+      dirty[tid] = cand_slot < 0;
+    }
+    __syncthreads();
+
+    double t = p.t0, dprev = 0.0;
+    u64 fired = 0;
+    int mu_prev = -1, stop = 0, status = RT_OK;
+    bool finishing = false;
+    int cur = 0;                         // staged-list buffer this firing publishes
+    // walker warp: what it has prepared for the likely next winner
+    int k2 = 0x7fffffff;                 //   runner-up of the last exchange
+    int pw_k = -1, pw_n = 0;             //   pre-walked reaction: its entries in [k0, k1) are in pw_d / pw_c
+    int4 pw_ent = make_int4(-1, 0, 0, 0);//   its stoich row (lanes 0..3)
+    bool sp_valid = false, sp_bad = false;  // speculative refreshes of pw_k in out_*[1 - cur], computed
+    u64 sp_state = 0;                    //   from X after firing number sp_state
+    long long sp_xn = 0;                 //   new count of the changed species of lane e < 4
+    int pf_k = -1;                       // exchange warp: candidate whose walk data was last prefetched
+
+    for (;;) {   // one iteration per firing, plus one closing pass
+      Cand best = none, extra = none;
+      if (is_stream) {
+        // ===== S1: advance and divide the candidate; also advance the reaction that fired
+        u64 mask = 0;
+        if (cand_slot >= 0) {
+          const int i = tid + cand_slot * NT;
+          const double a = sA[i];
+          const double tn = __dadd_rn(sT[i], __dmul_rn(a, dprev));
+          sT[i] = tn;
+          best.dt = waiting_time(sP[i], tn, a);
+          best.k = k0 + i;
+          mask = 1ull << cand_slot;
+        }
+        if (mu_prev >= k0 && mu_prev < k1 && (mu_prev - k0) % NT == tid) {
+          const int i = mu_prev - k0;
+          const u64 bit = 1ull << (i / NT);
+          if (!(mask & bit)) { sT[i] = __dadd_rn(sT[i], __dmul_rn(sA[i], dprev)); mask |= bit; }
+        }
+        advm[tid] = mask;
+      } else if (is_walker) {
+        // ===== walker warp: a-6, a-7, a-8 of the firing, and its refreshes (a-1)
+        if (lane == 0) ctx.p_k = -1;
+        int n = 0;
+        bool more = false;
+        Ranges rg;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { rg.lo[e] = 0; rg.end[e] = 0; }
+        uint32_t w_f = 0, w_e0 = 0;
+        int w_e = 0, w_ne = 0;
+        bool w_csr = false, hit = false;
+        if (mu_prev >= 0) {
+          if (lane == 0) {
+            if (mu_prev >= k0 && mu_prev < k1) {          // a-7: new internal firing time of mu (Eq.26)
+              uint32_t n1;
+              double pv;
+              if (ctx.spec_k == mu_prev) { n1 = ctx.spec_n; pv = ctx.spec_P; }
+              else {
+                n1 = nfire[mu_prev] + 1u;
+                const double e_new = exp_draw(p.seed, traj, (uint32_t)mu_prev, n1);
+                pv = resid ? -e_new : __dadd_rn(sP[mu_prev - k0], e_new);
+              }
+              nfire[mu_prev] = n1;
+              ctx.p_val = pv;
+              ctx.p_k = mu_prev;
+              ctx.spec_k = -1;
+            }
+            if (tracing && fired - 1 < p.trace_cap) {     // a-8
+              if (p.trace_mu) p.trace_mu[fired - 1] = mu_prev;
+              if (p.trace_t) p.trace_t[fired - 1] = t;
+            }
+          }
+          hit = sp_valid && pw_k == mu_prev && sp_state + 1 == fired;
+          if (hit) {
+            // the refreshes are already in out_*[cur]; X += v_mu (a-6) with the counts known in advance
+            if (sp_bad) { if (lane == 0) ctx.abort_local = 1; }
+            else if (lane < 4 && pw_ent.x >= 0) atomicMax(X + pw_ent.x, x_pack(fired, sp_xn));
+            n = pw_n;
+          } else {
+            int4 ent = make_int4(-1, 0, 0, 0);
+            if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(net.srow) + (size_t)mu_prev * 4 + lane);
+            w_csr = __shfl_sync(0xffffffffu, ent.x, 0) == -2;
+            if (!w_csr) {
+              const bool active = ent.x >= 0;
+              bool done = false;
+              long long xn = 0;
+              uint32_t lo = 0, hi = 0;
+              if (active && k1 > k0) { lo = (uint32_t)ent.z; hi = (uint32_t)ent.w; narrow_range(net, lo, hi, k0, k1); }
+              if (active) xn = x_peek(X, ent.x, ent.y, fired, net.xmax, done);
+              const bool bad = __any_sync(0xffffffffu, active && xn < 0);
+              if (bad) { if (lane == 0) ctx.abort_local = 1; }
+              else if (active && !done) atomicMax(X + ent.x, x_pack(fired, xn));
+              uint32_t acc = 0;
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                rg.lo[e] = __shfl_sync(0xffffffffu, lo, e);
+                acc += __shfl_sync(0xffffffffu, hi - lo, e);
+                rg.end[e] = acc;
+              }
+            } else {
+              // rows with more than 4 changed species: plain CSR walk (rare, correctness path)
+              w_e0 = __ldg(net.stoich_ptr + mu_prev);
+              w_ne = (int)(__ldg(net.stoich_ptr + mu_prev + 1) - w_e0);
+              bool bad_l = false;
+              for (int e = lane; e < w_ne; e += 32) {
+                bool done;
+                bad_l |= x_peek(X, __ldg(net.stoich_species + w_e0 + e), __ldg(net.stoich_v + w_e0 + e),
+                                fired, net.xmax, done) < 0;
+              }
+              if (__any_sync(0xffffffffu, bad_l)) {
+                if (lane == 0) ctx.abort_local = 1;
+              } else {
+                for (int e = lane; e < w_ne; e += 32) {
+                  bool done;
+                  const int j = __ldg(net.stoich_species + w_e0 + e);
+                  const long long xn = x_peek(X, j, __ldg(net.stoich_v + w_e0 + e), fired, net.xmax, done);
+                  if (!done) atomicMax(X + j, x_pack(fired, xn));
+                }
+              }
+              if (k1 <= k0) w_ne = 0;
+            }
+            __syncwarp();                          // this warp's X updates precede its reads below
+          }
+        }
+        // rounds: one, unless this CTA has more than kListCap refreshes
+        for (;;) {
+          if (!hit && mu_prev >= 0) {
+            n = 0;
+            if (!w_csr) {
+              more = walk_scan(net, rg, w_f, k0, k1, lane, n, list_d, out_a[cur]);
+            } else {
+              more = false;
+              while (w_e < w_ne) {
+                if (w_f == 0) {                    // entering species w_e: fetch its range
+                  const int j = __ldg(net.stoich_species + w_e0 + w_e);
+                  const uint2 rec = __ldg(reinterpret_cast<const uint2 *>(net.sp_rec) + j);
+                  uint32_t lo = rec.x, hi = rec.y;
+                  if (hi - lo > (uint32_t)net.big_deg) { lo = (uint32_t)__ldg(net.sp_big + j); hi = 0xffffffffu; }
+                  narrow_range(net, lo, hi, k0, k1);
+                  rg.lo[0] = lo;
+                  rg.end[0] = rg.end[1] = rg.end[2] = rg.end[3] = hi - lo;
+                }
+                more = walk_scan(net, rg, w_f, k0, k1, lane, n, list_d, out_a[cur]);
+                if (more) break;
+                w_e += 1;
+                w_f = 0;
+              }
+            }
+            walk_finish<false>(p, 1.0, X, lane, n, list_d, out_k[cur], out_a[cur]);
+          }
+          if (lane == 0) { ctx.list_n = n; ctx.list_buf = cur; ctx.more = more ? 1 : 0; }
+          if (!more) { named_arrive<NT + 32>(kBarStaged); break; }
+          named_sync<NT + 32>(kBarStaged);
+          named_sync<NT + 32>(kBarMore);           // the stream warps have consumed this round
+        }
+      }
+
+      if (is_stream) {
+        bool first_round = true;
+        for (;;) {
+          named_sync<NT + 32>(kBarStaged);
+          // ===== S2: apply the staged refreshes
+          const int n = ctx.list_n;
+          const bool more = ctx.more != 0;
+          const int *lk = out_k[ctx.list_buf];
+          const double *la = out_a[ctx.list_buf];
+          const int pk_now = ctx.p_k;
+          for (int i = tid; i < n; i += NT) {
+            const int k = lk[i];
+            const double a_new = la[i];
+            const int li = k - k0, o = li % NT;
+            const u64 bit = 1ull << (li / NT);
+            if (atomicOr(&refm[o], bit) & bit) continue;      // (a reaction reading two changed species is listed twice)
+            if (!(advm[o] & bit)) {                           // T_k += a_k dt with the OLD a_k, once
+              sT[li] = __dadd_rn(sT[li], __dmul_rn(sA[li], dprev));
+              atomicOr(&advm[o], bit);
+            }
+            sA[li] = a_new;
+            if (filter_unsafe(a_new)) ctx.any_odd = 1;
+            // A refreshed reaction invalidates its owner's proposal only if it IS that proposal;
+            // otherwise its new waiting time joins the reduction as one more candidate.
+            if (mybest_k[o] == k || mybest_k[o] == -3 || k == pk_now) {
+              dirty[o] = 1;
+            } else {
+              const double d = waiting_time(sP[li], sT[li], a_new);
+              if (cand_less(d, k, extra)) { extra.dt = d; extra.k = k; }
+            }
+          }
+          if (tid == 0 && first_round && pk_now >= 0) {
+            if (resid) sT[pk_now - k0] = ctx.p_val; else sP[pk_now - k0] = ctx.p_val;
+            dirty[(pk_now - k0) % NT] = 1;
+          }
+          if (!more) { named_sync<NT>(1); break; }
+          named_sync<NT + 32>(kBarMore);
+          first_round = false;
+        }
+        // ===== S3: exact re-scan of the threads without a valid candidate; the warp shares the work
+        unsigned stale_mask = __ballot_sync(0xffffffffu, dirty[tid] != 0);
+        if (dirty[tid]) dirty[tid] = 0;
+        while (stale_mask) {
+          const int L = __ffs(stale_mask) - 1;
+          stale_mask &= stale_mask - 1;
+          const int th = tid - lane + L;
+          const u64 m = advm[th];
+          Cand c = none;
+          for (int j = lane; j < nslot; j += 32) {
+            const int i = th + j * NT;
+            const double a = sA[i];
+            double tn = sT[i];
+            if (!((m >> j) & 1ull)) { tn = __dadd_rn(tn, __dmul_rn(a, dprev)); sT[i] = tn; }
+            const double d = waiting_time(sP[i], tn, a);
+            if (cand_less(d, k0 + i, c)) { c.dt = d; c.k = k0 + i; }
+          }
+          c = warp_lexmin(c);
+          __syncwarp();
+          if (lane == L) { best = c; advm[tid] = ~0ull; }
+        }
+        if (cand_less(extra.dt, extra.k, best)) best = extra;
+        // ===== S4: block argmin -> exchange warp
+        if (!finishing) {
+          best = warp_lexmin(best);
+          if (lane == 0) ctx.warp_part[warp] = best;
+          named_arrive<NT + 32>(kBarParts);
+        }
+        // ===== S5: the pass, while the exchange is in flight
+        cand_slot = pass_and_pick<NT>(tid, cnt_pad, sT, sP, sA, dprev, advm[tid], ctx.any_odd != 0);
+        mybest_k[tid] = cand_slot >= 0 ? k0 + tid + cand_slot * NT : -3;
+        if (cand_slot < 0) dirty[tid] = 1;
+        advm[tid] = 0;
+        refm[tid] = 0;
+      } else if (is_xw) {
+        if (!finishing) named_sync<NT + 32>(kBarParts);
+      }
+      if (ctx.abort_local) { status = RT_ERR_OVERFLOW; stop = 0; break; }
+      if (finishing) break;
+
+      // ---- a-3 argmin over the bundle
+      Cand win;
+      if (is_xw) {
+        Cand c = none;
+        if (lane < XW) c = ctx.warp_part[lane];
+        c = warp_lexmin(c);
+        const Cand mine = c;
+        Cand c2;
+        // While the exchange is in flight: if this CTA's candidate wins (it usually stays the candidate
+        // for many firings before it does), the CTA must redraw P_k (Philox + log, the longest serial
+        // piece of a firing).  Do it now, speculatively, once per candidate.
+        auto redraw = [&]() {
+          if (lane == 0 && mine.k < M && mine.k != ctx.spec_k && (p.prefetch & 2)) {
+            const uint32_t n1 = nfire[mine.k] + 1u;
+            const double e_new = exp_draw(p.seed, traj, (uint32_t)mine.k, n1);
+            ctx.spec_P = resid ? -e_new : __dadd_rn(sP[mine.k - k0], e_new);
+            ctx.spec_n = n1;
+            ctx.spec_k = mine.k;
+          }
+        };
+        exchange_partials<CLUSTER>(p, ctx.cl_slot, ctx.cl_bar, exch, r, gen, lane, c, c2, redraw);
+        if (lane == 0) { ctx.win = c; ctx.second_k = (c2.dt < INF) ? c2.k : 0x7fffffff; }
+        named_arrive<BLOCK>(kBarWin);
+        win = c;
+        // every CTA will need the candidate's stoich row and the dependency entries of its species,
+        // all DRAM-cold (each reaction fires rarely): pull them into L2, once per candidate
+        if (mine.k != pf_k && mine.k < M && (p.prefetch & 1)) {
+          pf_k = mine.k;
+          int4 ent = make_int4(-1, 0, 0, 0);
+          if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(net.srow) + (size_t)mine.k * 4 + lane);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int j = __shfl_sync(0xffffffffu, ent.x, e);
+            const uint32_t lo = (uint32_t)__shfl_sync(0xffffffffu, ent.z, e);
+            const uint32_t hi = (uint32_t)__shfl_sync(0xffffffffu, ent.w, e);
+            if (j >= 0 && hi != 0xffffffffu)
+              for (uint32_t i = lo + 4u * lane; i < hi; i += 128u)
+                prefetch_l2(reinterpret_cast<const char *>(net.dep) + (size_t)i * 32);
+          }
+        }
+      } else {
+        if (is_walker) {
+          // ===== walker: prepare the likely next winner k2 while the others reduce and exchange
+          // (1) its dependency entries in [k0, k1) (network data): row -> ranges -> entries
+          if ((p.prefetch & 4) && k2 != pw_k && k2 < M && k1 > k0) {
+            pw_k = -1;
+            int4 ent = make_int4(-1, 0, 0, 0);
+            if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(net.srow) + (size_t)k2 * 4 + lane);
+            if (__shfl_sync(0xffffffffu, ent.x, 0) != -2) {
+              uint32_t lo = 0, hi = 0;
+              if (ent.x >= 0) { lo = (uint32_t)ent.z; hi = (uint32_t)ent.w; narrow_range(net, lo, hi, k0, k1); }
+              Ranges rg;
+              uint32_t acc = 0;
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                rg.lo[e] = __shfl_sync(0xffffffffu, lo, e);
+                acc += __shfl_sync(0xffffffffu, hi - lo, e);
+                rg.end[e] = acc;
+              }
+              uint32_t f = 0;
+              int n = 0;
+              if (!walk_scan(net, rg, f, k0, k1, lane, n, pw_d, pw_c)) { pw_k = k2; pw_n = n; pw_ent = ent; }
+            }
+          }
+          // (2) its refreshes, computed from X as it will be after it fires: X now (this warp's own
+          // updates of every firing so far precede these loads: __syncwarp) plus its own v.  Another
+          // CTA of the bundle may already be one firing ahead (the exchange needs this CTA's exchange
+          // warp, not this warp): a word of version fired + 1 already holds that firing's change,
+          // which is k2's own if the guess is right (and if it is wrong the result is never used).
+          sp_valid = false;
+          if ((p.prefetch & 4) && pw_k >= 0 && pw_k == k2) {
+            __syncwarp();
+            int cj[4], cv[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              cj[e] = __shfl_sync(0xffffffffu, pw_ent.x, e);
+              cv[e] = __shfl_sync(0xffffffffu, pw_ent.y, e);
+            }
+            bool bad = false, general = false;
+            sp_xn = 0;
+            if (lane < 4 && pw_ent.x >= 0) {
+              const u64 w = __ldcg(X + pw_ent.x);
+              sp_xn = x_count(w) + (x_version(w) <= fired ? (long long)pw_ent.y : 0ll);
+              bad = sp_xn < 0 || sp_xn > net.xmax;
+            }
+            int *ok = out_k[1 - cur];
+            double *oa = out_a[1 - cur];
+            for (int i = lane; i < pw_n; i += 32) {
+              const int4 d = pw_d[i];
+              if (d.w & 0x10000) { general = true; continue; }   // > 2 reactants: not speculated
+              const u64 w1 = __ldcg(X + d.y);
+              const u64 w2 = __ldcg(X + (d.z >= 0 ? d.z : d.y));
+              long long x1 = x_count(w1), x2 = x_count(w2);
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                if (cj[e] == d.y && x_version(w1) <= fired) x1 += (long long)cv[e];
+                if (cj[e] == d.z && x_version(w2) <= fired) x2 += (long long)cv[e];
+              }
+              double a = __dmul_rn(pw_c[i], __ll2double_rn(binom(x1, d.w & 0xff)));
+              if (d.z >= 0) a = __dmul_rn(a, __ll2double_rn(binom(x2, (d.w >> 8) & 0xff)));
+              ok[i] = d.x;
+              oa[i] = a;
+            }
+            sp_bad = __any_sync(0xffffffffu, bad);
+            sp_valid = !__any_sync(0xffffffffu, general);
+            sp_state = fired;
+          }
+        }
+        named_sync<BLOCK>(kBarWin);
+        win = ctx.win;
+        if (is_walker) k2 = ctx.second_k;
+      }
+      gen += 1u;
+      cur ^= 1;
+      if (win.k == -2) return;
+
+      // ---- a-4 stop tests, identical in every thread of every CTA of the bundle
+      const double delta = win.dt;
+      if (delta == INF) { stop = RT_STOP_ABSORBED; break; }
+      if (p.t_end < INF && __dadd_rn(t, delta) > p.t_end) {
+        dprev = __dsub_rn(p.t_end, t);           // closing pass: T_k += a_k * (t_end - t), no firing
+        t = p.t_end;
+        mu_prev = -1;
+        stop = RT_STOP_T_END;
+        finishing = true;
+        continue;
+      }
+      if (fired >= kXMaxVersion) { status = RT_ERR_OVERFLOW; break; }
+      t = __dadd_rn(t, delta);
+      fired += 1;
+      mu_prev = win.k;
+      dprev = delta;
+      if (p.max_firings != 0 && fired == p.max_firings) {
+        stop = RT_STOP_MAX_FIRINGS;              // closing pass applies this firing's updates
+        finishing = true;
+      }
+    }
+
+    // ---- trajectory done: every CTA's X updates are visible bundle-wide after the fenced barrier
+    if (!bundle_barrier<BLOCK, CLUSTER>(exch, p.S, r, gen, p.err)) return;
+    if (!CLUSTER) gen += 1u;
+    for (int k = k0 + tid; k < k1; k += BLOCK) {
+      __stcg(T + k, sT[k - k0]); __stcg(P + k, sP[k - k0]); __stcg(A + k, sA[k - k0]);
+    }
+    if (p.x_out)
+      for (int j = r * BLOCK + tid; j < N; j += p.S * BLOCK)
+        p.x_out[it * (u64)N + (u64)j] = x_load(X, j);
+    if (r == 0 && tid == 0) {
+      rt_result res;
+      res.t = t; res.firings = fired; res.stop = stop; res.status = status;
+      p.res[it] = res;
+    }
+    if (tid == 0) { ctx.abort_local = 0; ctx.p_k = -1; ctx.any_odd = 0; ctx.spec_k = -1; }
+    if (is_stream) { dirty[tid] = 0; advm[tid] = 0; refm[tid] = 0; }
+    __syncthreads();
+  }
+}
+
+}  // namespace rt
