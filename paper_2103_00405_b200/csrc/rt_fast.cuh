@@ -46,6 +46,22 @@ constexpr int kFastHelperWarps = 2;
 constexpr int kBarMore = 5, kBarWin = 6;
 constexpr int kQTolUnits = 32;       // key margin, in units of the high word's last bit
 constexpr int kGuardShift = 29;      // high word of P - T may be at most this many binades below max(|P|, |T|)'s
+constexpr int kRepickPeriod = 8;     // a warp re-derives its threads' candidates at least this often
+
+// Per-thread 64-bit slot masks in shared memory, kept as two words so that a bit is set with a
+// native 32-bit shared-memory atomic.
+__device__ __forceinline__ u64 mask_load(const unsigned (*m)[2], int t) {
+  const uint2 v = *reinterpret_cast<const uint2 *>(m[t]);
+  return (u64)v.x | ((u64)v.y << 32);
+}
+__device__ __forceinline__ void mask_store(unsigned (*m)[2], int t, u64 v) {
+  *reinterpret_cast<uint2 *>(m[t]) = make_uint2((unsigned)v, (unsigned)(v >> 32));
+}
+// sets bit `slot` of thread t's mask; true if this call set it
+__device__ __forceinline__ bool mask_claim(unsigned (*m)[2], int t, int slot) {
+  const unsigned bit = 1u << (slot & 31);
+  return (atomicOr(&m[t][slot >> 5], bit) & bit) == 0u;
+}
 
 template <int BLOCK>
 struct FastCtx {
@@ -104,6 +120,23 @@ __device__ __forceinline__ int pass_and_pick(int tid, int cnt_pad, double *__res
   return decided ? s1 : -1;
 }
 
+// S5 of a thread that keeps its candidate: T_k += a_k dt for the reactions not yet advanced, nothing else
+// (24 instead of 32 bytes of shared-memory traffic per reaction, a third of the instructions).
+template <int NT>
+__device__ __forceinline__ void pass_advance(int tid, int cnt_pad, double *__restrict__ sT,
+                                             const double *__restrict__ sA, double dprev, u64 done) {
+  constexpr int U = kScanBatch;
+  int slot = 0;
+  for (int i = tid; i < cnt_pad; i += U * NT, slot += U) {
+    double a[U], t[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) { a[u] = sA[i + u * NT]; t[u] = sT[i + u * NT]; }
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+      if (!((done >> (slot + u)) & 1ull)) sT[i + u * NT] = __dadd_rn(t[u], __dmul_rn(a[u], dprev));
+  }
+}
+
 template <int BLOCK, bool CLUSTER>
 __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p) {
   constexpr int NT = BLOCK - 32 * kFastHelperWarps;   // stream threads
@@ -115,10 +148,12 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
   __shared__ int4 list_d[kListCap];
   __shared__ int4 pw_d[kListCap];                     // pre-walked dependency entries of reaction pw_k
   __shared__ double pw_c[kListCap];
-  __shared__ u64 advm[NT];                            // per stream thread: slots already advanced this firing
-  __shared__ u64 refm[NT];                            //                    slots whose refresh is claimed
+  __shared__ __align__(8) unsigned advm[NT][2];       // per stream thread: slots already advanced this firing
+  __shared__ __align__(8) unsigned refm[NT][2];       //                    slots whose refresh is claimed
   __shared__ int mybest_k[NT];                        // reaction each stream thread proposes (-3: none)
-  __shared__ unsigned char dirty[NT];
+  __shared__ double dcand[NT];                        //   and its exact waiting time for this firing
+  __shared__ unsigned char dirty[NT];                 // the thread's proposal is void: exact re-scan (S3)
+  __shared__ unsigned char repick[NT];                // the thread's candidate may have lost its margin
   extern __shared__ __align__(16) unsigned char dyn_smem[];
   const NetDev &net = p.net;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -155,7 +190,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
     mbar_init(smem_addr(&ctx.cl_bar[1]), 1u);
     mbar_fence_init();
   }
-  if (is_stream) { dirty[tid] = 0; advm[tid] = 0; refm[tid] = 0; mybest_k[tid] = -3; }
+  if (is_stream) { dirty[tid] = 0; repick[tid] = 0; mask_store(advm, tid, 0); mask_store(refm, tid, 0); mybest_k[tid] = -3; }
   __syncthreads();
   Cand none; none.dt = INF; none.k = 0x7fffffff;
 
@@ -226,7 +261,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           const u64 bit = 1ull << (i / NT);
           if (!(mask & bit)) { sT[i] = __dadd_rn(sT[i], __dmul_rn(sA[i], dprev)); mask |= bit; }
         }
-        advm[tid] = mask;
+        mask_store(advm, tid, mask);
+        dcand[tid] = best.dt;
       } else if (is_walker) {
         // ===== walker warp: a-6, a-7, a-8 of the firing, and its refreshes (a-1)
         if (lane == 0) ctx.p_k = -1;
@@ -238,34 +274,40 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         uint32_t w_f = 0, w_e0 = 0;
         int w_e = 0, w_ne = 0;
         bool w_csr = false, hit = false;
+        bool published = false;
         if (mu_prev >= 0) {
-          if (lane == 0) {
-            if (mu_prev >= k0 && mu_prev < k1) {          // a-7: new internal firing time of mu (Eq.26)
-              uint32_t n1;
-              double pv;
-              if (ctx.spec_k == mu_prev) { n1 = ctx.spec_n; pv = ctx.spec_P; }
-              else {
-                n1 = nfire[mu_prev] + 1u;
-                const double e_new = exp_draw(p.seed, traj, (uint32_t)mu_prev, n1);
-                pv = resid ? -e_new : __dadd_rn(sP[mu_prev - k0], e_new);
-              }
-              nfire[mu_prev] = n1;
-              ctx.p_val = pv;
-              ctx.p_k = mu_prev;
-              ctx.spec_k = -1;
+          if (lane == 0 && mu_prev >= k0 && mu_prev < k1) {   // a-7: new internal firing time of mu (Eq.26)
+            uint32_t n1;
+            double pv;
+            if (ctx.spec_k == mu_prev) { n1 = ctx.spec_n; pv = ctx.spec_P; }
+            else {
+              n1 = nfire[mu_prev] + 1u;
+              const double e_new = exp_draw(p.seed, traj, (uint32_t)mu_prev, n1);
+              pv = resid ? -e_new : __dadd_rn(sP[mu_prev - k0], e_new);
             }
-            if (tracing && fired - 1 < p.trace_cap) {     // a-8
-              if (p.trace_mu) p.trace_mu[fired - 1] = mu_prev;
-              if (p.trace_t) p.trace_t[fired - 1] = t;
-            }
+            nfire[mu_prev] = n1;
+            ctx.p_val = pv;
+            ctx.p_k = mu_prev;
+            ctx.spec_k = -1;
           }
           hit = sp_valid && pw_k == mu_prev && sp_state + 1 == fired;
           if (hit) {
-            // the refreshes are already in out_*[cur]; X += v_mu (a-6) with the counts known in advance
-            if (sp_bad) { if (lane == 0) ctx.abort_local = 1; }
-            else if (lane < 4 && pw_ent.x >= 0) atomicMax(X + pw_ent.x, x_pack(fired, sp_xn));
+            // the refreshes are already in out_*[cur]: publish them at once
             n = pw_n;
-          } else {
+            if (lane == 0) {
+              if (sp_bad) ctx.abort_local = 1;
+              ctx.list_n = n; ctx.list_buf = cur; ctx.more = 0;
+            }
+            named_arrive<NT + 32>(kBarStaged);
+            published = true;
+            // X += v_mu (a-6) with the counts known in advance
+            if (!sp_bad && lane < 4 && pw_ent.x >= 0) atomicMax(X + pw_ent.x, x_pack(fired, sp_xn));
+          }
+          if (lane == 0 && tracing && fired - 1 < p.trace_cap) {     // a-8
+            if (p.trace_mu) p.trace_mu[fired - 1] = mu_prev;
+            if (p.trace_t) p.trace_t[fired - 1] = t;
+          }
+          if (!hit) {
             int4 ent = make_int4(-1, 0, 0, 0);
             if (lane < 4) ent = __ldg(reinterpret_cast<const int4 *>(net.srow) + (size_t)mu_prev * 4 + lane);
             w_csr = __shfl_sync(0xffffffffu, ent.x, 0) == -2;
@@ -312,8 +354,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           }
         }
         // rounds: one, unless this CTA has more than kListCap refreshes
-        for (;;) {
-          if (!hit && mu_prev >= 0) {
+        while (!published) {
+          if (mu_prev >= 0) {
             n = 0;
             if (!w_csr) {
               more = walk_scan(net, rg, w_f, k0, k1, lane, n, list_d, out_a[cur]);
@@ -357,13 +399,10 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           for (int i = tid; i < n; i += NT) {
             const int k = lk[i];
             const double a_new = la[i];
-            const int li = k - k0, o = li % NT;
-            const u64 bit = 1ull << (li / NT);
-            if (atomicOr(&refm[o], bit) & bit) continue;      // (a reaction reading two changed species is listed twice)
-            if (!(advm[o] & bit)) {                           // T_k += a_k dt with the OLD a_k, once
+            const int li = k - k0, o = li % NT, slot = li / NT;
+            if (!mask_claim(refm, o, slot)) continue;         // (a reaction reading two changed species is listed twice)
+            if (mask_claim(advm, o, slot))                    // T_k += a_k dt with the OLD a_k, once
               sT[li] = __dadd_rn(sT[li], __dmul_rn(sA[li], dprev));
-              atomicOr(&advm[o], bit);
-            }
             sA[li] = a_new;
             if (filter_unsafe(a_new)) ctx.any_odd = 1;
             // A refreshed reaction invalidates its owner's proposal only if it IS that proposal;
@@ -373,6 +412,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
             } else {
               const double d = waiting_time(sP[li], sT[li], a_new);
               if (cand_less(d, k, extra)) { extra.dt = d; extra.k = k; }
+              // the owner keeps its candidate only while every other reaction of it stays clear of it
+              if (!(d > __dmul_rn(dcand[o], 1.0 + 0x1.0p-14))) repick[o] = 1;
             }
           }
           if (tid == 0 && first_round && pk_now >= 0) {
@@ -385,12 +426,13 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         }
         // ===== S3: exact re-scan of the threads without a valid candidate; the warp shares the work
         unsigned stale_mask = __ballot_sync(0xffffffffu, dirty[tid] != 0);
+        bool pick = dirty[tid] != 0 || repick[tid] != 0 || cand_slot < 0;
         if (dirty[tid]) dirty[tid] = 0;
         while (stale_mask) {
           const int L = __ffs(stale_mask) - 1;
           stale_mask &= stale_mask - 1;
           const int th = tid - lane + L;
-          const u64 m = advm[th];
+          const u64 m = mask_load(advm, th);
           Cand c = none;
           for (int j = lane; j < nslot; j += 32) {
             const int i = th + j * NT;
@@ -402,7 +444,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           }
           c = warp_lexmin(c);
           __syncwarp();
-          if (lane == L) { best = c; advm[tid] = ~0ull; }
+          if (lane == L) { best = c; mask_store(advm, tid, ~0ull); }
         }
         if (cand_less(extra.dt, extra.k, best)) best = extra;
         // ===== S4: block argmin -> exchange warp
@@ -412,11 +454,20 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           named_arrive<NT + 32>(kBarParts);
         }
         // ===== S5: the pass, while the exchange is in flight
-        cand_slot = pass_and_pick<NT>(tid, cnt_pad, sT, sP, sA, dprev, advm[tid], ctx.any_odd != 0);
-        mybest_k[tid] = cand_slot >= 0 ? k0 + tid + cand_slot * NT : -3;
-        if (cand_slot < 0) dirty[tid] = 1;
-        advm[tid] = 0;
-        refm[tid] = 0;
+        // A thread keeps its candidate (and only advances) unless the candidate is void or may have
+        // lost its margin; every kRepickPeriod firings the warp re-derives all of them, which bounds
+        // the age of a candidate (the lag argument of the header needs age * 2 + 7 < kQTolUnits units).
+        pick = pick || (((unsigned)fired + (unsigned)warp) % kRepickPeriod == 0u);
+        if (__any_sync(0xffffffffu, pick)) {
+          cand_slot = pass_and_pick<NT>(tid, cnt_pad, sT, sP, sA, dprev, mask_load(advm, tid), ctx.any_odd != 0);
+          mybest_k[tid] = cand_slot >= 0 ? k0 + tid + cand_slot * NT : -3;
+          if (cand_slot < 0) dirty[tid] = 1;
+        } else {
+          pass_advance<NT>(tid, cnt_pad, sT, sA, dprev, mask_load(advm, tid));
+        }
+        repick[tid] = 0;
+        mask_store(advm, tid, 0);
+        mask_store(refm, tid, 0);
       } else if (is_xw) {
         if (!finishing) named_sync<NT + 32>(kBarParts);
       }
@@ -576,7 +627,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
       p.res[it] = res;
     }
     if (tid == 0) { ctx.abort_local = 0; ctx.p_k = -1; ctx.any_odd = 0; ctx.spec_k = -1; }
-    if (is_stream) { dirty[tid] = 0; advm[tid] = 0; refm[tid] = 0; }
+    if (is_stream) { dirty[tid] = 0; repick[tid] = 0; mask_store(advm, tid, 0); mask_store(refm, tid, 0); }
     __syncthreads();
   }
 }
