@@ -38,7 +38,7 @@ namespace {
 constexpr int kBlockSmem = RT_BLOCK_SMEM;
 constexpr int kBlockGlobal = RT_BLOCK_GLOBAL;
 constexpr int kBlockFast = RT_BLOCK_FAST;                      // candidate-first kernel (rt_fast.cuh)
-constexpr size_t kSmemStateBytesFast = 204 * 1024;             // (its static shared memory is larger)
+constexpr size_t kSmemStateBytesFast = 203 * 1024;             // (its static shared memory is larger)
 constexpr int kThreadKernelMaxM = 64; // one-thread-per-trajectory path: M, N at most this
 constexpr int kMinPairsPerCta = 256;  // do not spread a trajectory thinner than this
 constexpr int kBigDeg = 64;           // species read by more reactions than this get a block-offset table

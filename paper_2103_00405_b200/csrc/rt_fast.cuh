@@ -44,9 +44,9 @@ namespace rt {
 
 constexpr int kFastHelperWarps = 2;
 constexpr int kBarMore = 5, kBarWin = 6;
-constexpr int kQTolUnits = 32;       // key margin, in units of the high word's last bit
+constexpr int kQTolUnits = 64;       // key margin, in units of the high word's last bit
 constexpr int kGuardShift = 29;      // high word of P - T may be at most this many binades below max(|P|, |T|)'s
-constexpr int kRepickPeriod = 8;     // a warp re-derives its threads' candidates at least this often
+constexpr int kRepickPeriod = 24;    // a warp re-derives its threads' candidates at least this often
 
 // Per-thread 64-bit slot masks in shared memory, kept as two words so that a bit is set with a
 // native 32-bit shared-memory atomic.
@@ -69,11 +69,6 @@ struct FastCtx {
   Cand win;
   int second_k;
   int abort_local, list_n, list_buf, more, any_odd;
-  int p_k;                // reaction whose P was redrawn (or -1), and its new value
-  double p_val;
-  int spec_k;             // exchange warp -> walker: precomputed redraw of this CTA's candidate
-  uint32_t spec_n;
-  double spec_P;
   alignas(16) u64 cl_slot[2][kMaxClusterCtas][2];
   alignas(8) u64 cl_bar[2];
 };
@@ -154,6 +149,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
   __shared__ double dcand[NT];                        //   and its exact waiting time for this firing
   __shared__ unsigned char dirty[NT];                 // the thread's proposal is void: exact re-scan (S3)
   __shared__ unsigned char repick[NT];                // the thread's candidate may have lost its margin
+  __shared__ int newcand[NT];                         // a refreshed reaction clearly below the thread's candidate (slot, or -1)
   extern __shared__ __align__(16) unsigned char dyn_smem[];
   const NetDev &net = p.net;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -182,15 +178,15 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
 
   uint32_t gen = 0;
   if (tid == 0) {
-    ctx.abort_local = 0; ctx.list_n = 0; ctx.list_buf = 0; ctx.more = 0; ctx.p_k = -1; ctx.any_odd = 0;
-    ctx.spec_k = -1; ctx.second_k = 0x7fffffff;
+    ctx.abort_local = 0; ctx.list_n = 0; ctx.list_buf = 0; ctx.more = 0; ctx.any_odd = 0;
+    ctx.second_k = 0x7fffffff;
   }
   if (CLUSTER && tid == 0) {
     mbar_init(smem_addr(&ctx.cl_bar[0]), 1u);
     mbar_init(smem_addr(&ctx.cl_bar[1]), 1u);
     mbar_fence_init();
   }
-  if (is_stream) { dirty[tid] = 0; repick[tid] = 0; mask_store(advm, tid, 0); mask_store(refm, tid, 0); mybest_k[tid] = -3; }
+  if (is_stream) { dirty[tid] = 0; repick[tid] = 0; newcand[tid] = -1; mask_store(advm, tid, 0); mask_store(refm, tid, 0); mybest_k[tid] = -3; }
   __syncthreads();
   Cand none; none.dt = INF; none.k = 0x7fffffff;
 
@@ -241,6 +237,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
     u64 sp_state = 0;                    //   from X after firing number sp_state
     long long sp_xn = 0;                 //   new count of the changed species of lane e < 4
     int pf_k = -1;                       // exchange warp: candidate whose walk data was last prefetched
+    int spec_k = -1;                     // stream thread: the precomputed redraw of its candidate:
+    uint32_t spec_n = 0u;                //   its new firing count and
+    double spec_P = 0.0;                 //   new internal firing time P_k + E(seed, traj, k, n)
 
     for (;;) {   // one iteration per firing, plus one closing pass
       Cand best = none, extra = none;
@@ -257,15 +256,30 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           mask = 1ull << cand_slot;
         }
         if (mu_prev >= k0 && mu_prev < k1 && (mu_prev - k0) % NT == tid) {
+          // a-7: this thread owns the reaction that fired: new internal firing time (Eq.26), as a rule
+          // precomputed when the reaction became the thread's candidate (S5)
           const int i = mu_prev - k0;
           const u64 bit = 1ull << (i / NT);
-          if (!(mask & bit)) { sT[i] = __dadd_rn(sT[i], __dmul_rn(sA[i], dprev)); mask |= bit; }
+          if (spec_k != mu_prev) {
+            spec_n = nfire[mu_prev] + 1u;
+            const double e_new = exp_draw(p.seed, traj, (uint32_t)mu_prev, spec_n);
+            spec_P = resid ? -e_new : __dadd_rn(sP[i], e_new);
+          }
+          if (resid) {
+            sT[i] = spec_P;                              // Table 3: R_mu = ln(1/r), kept as T = -R
+          } else {
+            if (!(mask & bit)) sT[i] = __dadd_rn(sT[i], __dmul_rn(sA[i], dprev));
+            sP[i] = spec_P;
+          }
+          mask |= bit;
+          nfire[mu_prev] = spec_n;
+          spec_k = -1;
+          dirty[tid] = 1;                                // its proposal (if it was mu) is void
         }
         mask_store(advm, tid, mask);
         dcand[tid] = best.dt;
       } else if (is_walker) {
-        // ===== walker warp: a-6, a-7, a-8 of the firing, and its refreshes (a-1)
-        if (lane == 0) ctx.p_k = -1;
+        // ===== walker warp: a-6 of the firing and its refreshes (a-1)
         int n = 0;
         bool more = false;
         Ranges rg;
@@ -276,20 +290,6 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         bool w_csr = false, hit = false;
         bool published = false;
         if (mu_prev >= 0) {
-          if (lane == 0 && mu_prev >= k0 && mu_prev < k1) {   // a-7: new internal firing time of mu (Eq.26)
-            uint32_t n1;
-            double pv;
-            if (ctx.spec_k == mu_prev) { n1 = ctx.spec_n; pv = ctx.spec_P; }
-            else {
-              n1 = nfire[mu_prev] + 1u;
-              const double e_new = exp_draw(p.seed, traj, (uint32_t)mu_prev, n1);
-              pv = resid ? -e_new : __dadd_rn(sP[mu_prev - k0], e_new);
-            }
-            nfire[mu_prev] = n1;
-            ctx.p_val = pv;
-            ctx.p_k = mu_prev;
-            ctx.spec_k = -1;
-          }
           hit = sp_valid && pw_k == mu_prev && sp_state + 1 == fired;
           if (hit) {
             // the refreshes are already in out_*[cur]: publish them at once
@@ -302,10 +302,6 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
             published = true;
             // X += v_mu (a-6) with the counts known in advance
             if (!sp_bad && lane < 4 && pw_ent.x >= 0) atomicMax(X + pw_ent.x, x_pack(fired, sp_xn));
-          }
-          if (lane == 0 && tracing && fired - 1 < p.trace_cap) {     // a-8
-            if (p.trace_mu) p.trace_mu[fired - 1] = mu_prev;
-            if (p.trace_t) p.trace_t[fired - 1] = t;
           }
           if (!hit) {
             int4 ent = make_int4(-1, 0, 0, 0);
@@ -386,8 +382,12 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         }
       }
 
+      if (is_xw && lane == 0 && mu_prev >= 0 && tracing && fired - 1 < p.trace_cap) {   // a-8
+        if (p.trace_mu) p.trace_mu[fired - 1] = mu_prev;
+        if (p.trace_t) p.trace_t[fired - 1] = t;
+      }
+
       if (is_stream) {
-        bool first_round = true;
         for (;;) {
           named_sync<NT + 32>(kBarStaged);
           // ===== S2: apply the staged refreshes
@@ -395,7 +395,6 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           const bool more = ctx.more != 0;
           const int *lk = out_k[ctx.list_buf];
           const double *la = out_a[ctx.list_buf];
-          const int pk_now = ctx.p_k;
           for (int i = tid; i < n; i += NT) {
             const int k = lk[i];
             const double a_new = la[i];
@@ -407,43 +406,70 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
             if (filter_unsafe(a_new)) ctx.any_odd = 1;
             // A refreshed reaction invalidates its owner's proposal only if it IS that proposal;
             // otherwise its new waiting time joins the reduction as one more candidate.
-            if (mybest_k[o] == k || mybest_k[o] == -3 || k == pk_now) {
+            if (mybest_k[o] == k || mybest_k[o] == -3 || k == mu_prev) {
               dirty[o] = 1;
             } else {
-              const double d = waiting_time(sP[li], sT[li], a_new);
+              const double pk = sP[li], tk = sT[li];
+              const double d = waiting_time(pk, tk, a_new);
               if (cand_less(d, k, extra)) { extra.dt = d; extra.k = k; }
-              // the owner keeps its candidate only while every other reaction of it stays clear of it
-              if (!(d > __dmul_rn(dcand[o], 1.0 + 0x1.0p-14))) repick[o] = 1;
+              // The owner keeps its candidate while every other reaction of it stays clear of it (2^-13
+              // relative: 256 key units).  A refreshed reaction clearly BELOW the candidate simply becomes
+              // the candidate (everything else is above the old one); anything in between, a second such
+              // reaction, or one outside the cancellation guard sends the owner to a full re-pick.
+              const double dc = dcand[o];
+              if (!(d > __dmul_rn(dc, 1.0 + 0x1.0p-13))) {
+                const bool guard = __double2hiint(__dsub_rn(pk, tk)) + (kGuardShift << 20) >=
+                                   max(__double2hiint(pk) & 0x7fffffff, __double2hiint(tk) & 0x7fffffff);
+                if (d < __dmul_rn(dc, 1.0 - 0x1.0p-13) && d > 0.0 && guard && atomicCAS(&newcand[o], -1, slot) == -1) {}
+                else repick[o] = 1;
+              }
             }
-          }
-          if (tid == 0 && first_round && pk_now >= 0) {
-            if (resid) sT[pk_now - k0] = ctx.p_val; else sP[pk_now - k0] = ctx.p_val;
-            dirty[(pk_now - k0) % NT] = 1;
           }
           if (!more) { named_sync<NT>(1); break; }
           named_sync<NT + 32>(kBarMore);
-          first_round = false;
         }
         // ===== S3: exact re-scan of the threads without a valid candidate; the warp shares the work
         unsigned stale_mask = __ballot_sync(0xffffffffu, dirty[tid] != 0);
+        const int n_stale = __popc(stale_mask);
         bool pick = dirty[tid] != 0 || repick[tid] != 0 || cand_slot < 0;
         if (dirty[tid]) dirty[tid] = 0;
+        // Lane l takes slots l and l + 32 of the stale thread: advance, integer keys (as in the pass),
+        // then exact divisions only for the slots whose key is within kQTolUnits of the smallest --
+        // no other slot can hold the exact minimum.  Keys are not trusted (everything is divided) when
+        // the smallest is outside [2^-100, 2^100] (zero or negative residuals, NaN) or under any_odd.
+        int sq0 = 0x7fffffff, sq1 = 0x7fffffff, sm1 = 0x7fffffff;   // (kept for S5: the keys, their minimum,
+        Cand swin = none;                                            //  the exact winner, the stale lane)
+        int sL = -1;
+        bool sguard = true;
         while (stale_mask) {
           const int L = __ffs(stale_mask) - 1;
           stale_mask &= stale_mask - 1;
           const int th = tid - lane + L;
           const u64 m = mask_load(advm, th);
+          const int j0 = lane, j1 = lane + 32;
+          const bool h0 = j0 < nslot, h1 = j1 < nslot;
+          const int i0 = th + j0 * NT, i1 = th + j1 * NT;
+          double a0 = 0.0, p0 = 1.0, t0 = 0.0, a1 = 0.0, p1 = 1.0, t1 = 0.0;
+          if (h0) { a0 = sA[i0]; p0 = sP[i0]; t0 = sT[i0]; }
+          if (h1) { a1 = sA[i1]; p1 = sP[i1]; t1 = sT[i1]; }
+          if (h0 && !((m >> j0) & 1ull)) { t0 = __dadd_rn(t0, __dmul_rn(a0, dprev)); sT[i0] = t0; }
+          if (h1 && !((m >> j1) & 1ull)) { t1 = __dadd_rn(t1, __dmul_rn(a1, dprev)); sT[i1] = t1; }
+          sguard = true;
+          sq0 = q_key(p0, t0, a0, sguard);
+          sq1 = q_key(p1, t1, a1, sguard);
+          sm1 = __reduce_min_sync(0xffffffffu, min(sq0, sq1));
+          const bool trust = ctx.any_odd == 0 && sm1 >= ((1023 - 100) << 20) && sm1 <= ((1023 + 100) << 20);
+          const int lim = trust ? sm1 + kQTolUnits : 0x7fffffff;
           Cand c = none;
-          for (int j = lane; j < nslot; j += 32) {
-            const int i = th + j * NT;
-            const double a = sA[i];
-            double tn = sT[i];
-            if (!((m >> j) & 1ull)) { tn = __dadd_rn(tn, __dmul_rn(a, dprev)); sT[i] = tn; }
-            const double d = waiting_time(sP[i], tn, a);
-            if (cand_less(d, k0 + i, c)) { c.dt = d; c.k = k0 + i; }
+          if (h0 && sq0 <= lim) { c.dt = waiting_time(p0, t0, a0); c.k = k0 + i0; }
+          if (h1 && sq1 <= lim) {
+            const double d = waiting_time(p1, t1, a1);
+            if (cand_less(d, k0 + i1, c)) { c.dt = d; c.k = k0 + i1; }
           }
           c = warp_lexmin(c);
           __syncwarp();
+          swin = c; sL = L;
+          if (!trust) sguard = false;
           if (lane == L) { best = c; mask_store(advm, tid, ~0ull); }
         }
         if (cand_less(extra.dt, extra.k, best)) best = extra;
@@ -457,6 +483,26 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         // A thread keeps its candidate (and only advances) unless the candidate is void or may have
         // lost its margin; every kRepickPeriod firings the warp re-derives all of them, which bounds
         // the age of a candidate (the lag argument of the header needs age * 2 + 7 < kQTolUnits units).
+        if (n_stale == 1) {
+          // The re-scan decides the stale thread's new candidate as the pass would: the exact winner,
+          // if every other key is clear of the smallest and the cancellation guard holds.
+          const int wslot = (swin.k - k0 - (tid - lane + sL)) / NT;      // slot of the winner
+          const int e0 = (wslot == lane) ? 0x7fffffff : sq0;
+          const int e1 = (wslot == lane + 32) ? 0x7fffffff : sq1;
+          const int sm2 = __reduce_min_sync(0xffffffffu, min(e0, e1));
+          const bool ok = __all_sync(0xffffffffu, sguard) && swin.k < M && sm2 > sm1 + kQTolUnits;
+          if (lane == sL && ok && !repick[tid]) {
+            cand_slot = wslot;
+            mybest_k[tid] = swin.k;
+            pick = false;
+            newcand[tid] = -1;                       // (the re-scan has seen every refreshed reaction)
+          }
+        }
+        if (!pick && newcand[tid] >= 0) {            // (S2) a refreshed reaction took over as the candidate
+          cand_slot = newcand[tid];
+          mybest_k[tid] = k0 + tid + cand_slot * NT;
+        }
+        newcand[tid] = -1;
         pick = pick || (((unsigned)fired + (unsigned)warp) % kRepickPeriod == 0u);
         if (__any_sync(0xffffffffu, pick)) {
           cand_slot = pass_and_pick<NT>(tid, cnt_pad, sT, sP, sA, dprev, mask_load(advm, tid), ctx.any_odd != 0);
@@ -468,6 +514,14 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         repick[tid] = 0;
         mask_store(advm, tid, 0);
         mask_store(refm, tid, 0);
+        // If the candidate fires, this thread must redraw its P_k: Philox + log, the longest serial piece
+        // of a firing.  Do it now, off the critical path, once per candidate.
+        if (cand_slot >= 0 && mybest_k[tid] != spec_k && (p.prefetch & 2)) {
+          spec_k = mybest_k[tid];
+          spec_n = nfire[spec_k] + 1u;
+          const double e_new = exp_draw(p.seed, traj, (uint32_t)spec_k, spec_n);
+          spec_P = resid ? -e_new : __dadd_rn(sP[spec_k - k0], e_new);
+        }
       } else if (is_xw) {
         if (!finishing) named_sync<NT + 32>(kBarParts);
       }
@@ -482,19 +536,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         c = warp_lexmin(c);
         const Cand mine = c;
         Cand c2;
-        // While the exchange is in flight: if this CTA's candidate wins (it usually stays the candidate
-        // for many firings before it does), the CTA must redraw P_k (Philox + log, the longest serial
-        // piece of a firing).  Do it now, speculatively, once per candidate.
-        auto redraw = [&]() {
-          if (lane == 0 && mine.k < M && mine.k != ctx.spec_k && (p.prefetch & 2)) {
-            const uint32_t n1 = nfire[mine.k] + 1u;
-            const double e_new = exp_draw(p.seed, traj, (uint32_t)mine.k, n1);
-            ctx.spec_P = resid ? -e_new : __dadd_rn(sP[mine.k - k0], e_new);
-            ctx.spec_n = n1;
-            ctx.spec_k = mine.k;
-          }
-        };
-        exchange_partials<CLUSTER>(p, ctx.cl_slot, ctx.cl_bar, exch, r, gen, lane, c, c2, redraw);
+        exchange_partials<CLUSTER>(p, ctx.cl_slot, ctx.cl_bar, exch, r, gen, lane, c, c2);
         if (lane == 0) { ctx.win = c; ctx.second_k = (c2.dt < INF) ? c2.k : 0x7fffffff; }
         named_arrive<BLOCK>(kBarWin);
         win = c;
@@ -626,8 +668,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
       res.t = t; res.firings = fired; res.stop = stop; res.status = status;
       p.res[it] = res;
     }
-    if (tid == 0) { ctx.abort_local = 0; ctx.p_k = -1; ctx.any_odd = 0; ctx.spec_k = -1; }
-    if (is_stream) { dirty[tid] = 0; repick[tid] = 0; mask_store(advm, tid, 0); mask_store(refm, tid, 0); }
+    if (tid == 0) { ctx.abort_local = 0; ctx.any_odd = 0; }
+    if (is_stream) { dirty[tid] = 0; repick[tid] = 0; newcand[tid] = -1; mask_store(advm, tid, 0); mask_store(refm, tid, 0); }
     __syncthreads();
   }
 }
