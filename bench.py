@@ -31,15 +31,25 @@ import rt_workloads as W
 METRIC = "reaction firings/sec on 1 B200 at M=10^6 (+ % of HBM roofline per firing)"
 UNIT = "firings/s"
 BYTES_PER_REACTION_FIRING = 32   # read T, P, a; write T
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the bundle kernel, from the
-# `ncu --set full` capture of this command (profiles/r1_v7_bundle_kernel.md): 51.56 MB + 2.73 MB.
-# Far BELOW the algorithmic bytes: at M = 1e6 the (T,P,a) state lives in shared memory.
-NCU_TRAFFIC = {"cfg4": {"bytes": 54284800, "source": "profiles/r1_v7_bundle_kernel.md (ncu --set full, one launch)"}}
-# Small-network ensembles (cfg1, cfg2: one thread per trajectory, state in shared memory) are bound
-# by plain ALU issue, not memory.  Thread instructions per trajectory-step, from
-# `ncu --metrics smsp__thread_inst_executed.sum` over a whole launch:
-THREAD_INSTR_PER_STEP = {"cfg1": 382.0, "cfg2": 511.2}
-THREAD_INSTR_SOURCE = "profiles/r1_thread_kernel.md (ncu smsp__thread_inst_executed.sum / steps of one launch)"
+# Counters that a timed run cannot measure (DRAM bytes, shared-memory wavefronts, thread instructions)
+# come from the committed ncu captures of THIS command line, one row per workload:
+# profiles/r2_ncu_counters.csv (commands and commit in profiles/r2_ncu_counters.md).
+NCU_COUNTERS_CSV = os.path.join(ROOT, "profiles", "r2_ncu_counters.csv")
+
+
+def ncu_counters(workload):
+    """Row of profiles/r2_ncu_counters.csv for `workload` (dict of str), or None."""
+    import csv
+    try:
+        with open(NCU_COUNTERS_CSV, newline="") as f:
+            for row in csv.DictReader(f):
+                if row.get("workload") == workload:
+                    return row
+    except OSError:
+        pass
+    return None
+
+
 # the other BASELINE.json configs, reported in the same JSON line under "secondary"
 SECONDARY = ["cfg5a", "cfg5b", "cfg3", "cfg2"]
 SECONDARY_STEPS = 2
@@ -313,25 +323,32 @@ def measure(rt, torch, dist, args, workload, steps, warmup, rank, world, local, 
             "us_per_firing": us_per_firing, "ensemble_path": model.info("ensemble_path"),
             "formulation": "residual (Table 3)" if formulation else "(T, P) internal time",
             "rate_breakpoints": breakpoints}
-        if workload in THREAD_INSTR_PER_STEP:
+        ctr = ncu_counters(workload)
+        src = ("profiles/r2_ncu_counters.csv (ncu --set full, one launch of this command at commit "
+               + ctr["commit"] + ")") if ctr else None
+        if model.info("ensemble_path") == 1:
             # one thread per trajectory, state in shared memory: plain ALU issue is the bound
-            ginstr = THREAD_INSTR_PER_STEP[workload] * fired_local / kernel_s / 1e9
+            ips = float(ctr["thread_inst_executed"]) / float(ctr["steps_per_launch"]) if ctr else None
+            ginstr = ips * fired_local / kernel_s / 1e9 if ips else None
             out["roofline"] = {"bound": "alu", "achieved": ginstr, "peak": ALU_PEAK_GINSTR,
-                               "unit": "Ginstr/s", "frac": ginstr / ALU_PEAK_GINSTR, "traffic": None,
-                               "kernel": "rt_thread_kernel",
+                               "unit": "Ginstr/s", "frac": ginstr / ALU_PEAK_GINSTR if ginstr else None,
+                               "traffic": None, "kernel": "rt_thread_kernel",
                                "peak_source": "148 SMs x 4 schedulers x 32 lanes x 1.965 GHz (DESIGN.md 7)",
-                               "thread_instructions_per_step": THREAD_INSTR_PER_STEP[workload],
-                               "thread_instructions_source": THREAD_INSTR_SOURCE}
+                               "thread_instructions_per_step": ips, "thread_instructions_source": src}
         else:
             # residual (Table 3) form: T and a read, T written -- no P: 24 bytes per reaction
             bpr = 24 if formulation else BYTES_PER_REACTION_FIRING
             alg_bytes = bpr * M * fired_local
             achieved = alg_bytes / kernel_s / 1e9
-            tr = NCU_TRAFFIC.get(workload)
+            traffic = None
+            if ctr and int(ctr["steps_per_launch"]) > 0:
+                # DRAM bytes of the captured launch, scaled if this run fires a different number
+                traffic = (float(ctr["dram_bytes_read"]) + float(ctr["dram_bytes_write"])) * \
+                          fired_local / float(ctr["steps_per_launch"])
+            kernel = "rt_fast_kernel" if model.info("pipeline") else "rt_bundle_kernel"
             roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                    "frac": achieved / peak, "traffic": tr["bytes"] if tr else None,
-                    "traffic_source": tr["source"] if tr else None,
-                    "kernel": "rt_bundle_kernel", "peak_source": peak_src,
+                    "frac": achieved / peak, "traffic": traffic, "traffic_source": src,
+                    "kernel": kernel, "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": alg_bytes,
                     "frac_of_8TBs_nominal": achieved / 8000.0}
             if smem:
@@ -340,10 +357,17 @@ def measure(rt, torch, dist, args, workload, steps, warmup, rank, world, local, 
                 # one bundle's queue; aggregate bytes per second is what the shared memories deliver
                 roof.update(smem_roofline(M, kernel_s / max(fired_local, 1), sm_mhz,
                                           model.info("num_sms"), bpr))
-                roof["note"] = ("state (T,P,a) resident in shared memory: `achieved` is algorithmic bytes "
-                                "per second, not DRAM throughput (see `traffic`); the binding resource is "
-                                "shared-memory bandwidth + the per-firing latency chain: `smem_frac` "
-                                "(DESIGN.md 7)")
+                if ctr and ctr.get("smem_wavefronts"):
+                    # measured shared-memory traffic: wavefronts x 128 B of the captured launch
+                    smem_bytes = float(ctr["smem_wavefronts"]) * 128.0 / float(ctr["steps_per_launch"])
+                    roof["smem_bytes_per_firing_measured"] = smem_bytes
+                    roof["smem_bytes_per_firing_algorithmic"] = bpr * M
+                roof["bound_actual"] = "latency (per-firing dependency chain) + shared-memory bandwidth"
+                roof["note"] = ("state (T,P,a) resident in shared memory: `achieved` is ALGORITHMIC bytes per "
+                                "second (north_star's definition), not DRAM throughput (see `traffic`); a "
+                                "fraction above 1 only says the state never leaves the chip.  What binds is "
+                                "the per-firing latency chain (exchange + refresh) and shared-memory "
+                                "bandwidth: `smem_frac` (DESIGN.md 7)")
             else:
                 roof["note"] = "state streamed from global memory: DRAM traffic = algorithmic bytes"
             out["roofline"] = roof

@@ -254,7 +254,7 @@ Plan plan_bundles_for(rt_model *m, u64 n_traj, bool fast) {
   const int s_thin = std::max(1, (pairs_total + kMinPairsPerCta - 1) / kMinPairsPerCta);
   const bool may_cluster = m->opt_exchange != 1 && m->opt_state_mode != 1;
   int S, B = 0;
-  bool cluster = false;
+  bool cluster = false, force_l2 = false;
   if (m->opt_bundle_ctas > 0) {
     S = std::min(m->opt_bundle_ctas, sms);
   } else if (n_traj <= 1) {
@@ -268,17 +268,31 @@ Plan plan_bundles_for(rt_model *m, u64 n_traj, bool fast) {
     S = (int)std::max<u64>(1, (u64)sms / n_traj);       // many: as many bundles as fit ...
     if (m->opt_state_mode != 1 && S < s_fit && s_fit <= sms) S = s_fit;   // ... with on-chip state
     S = std::min(S, s_thin);
-    if (may_cluster && S >= 2 && S <= rt::kMaxClusterCtas && S >= s_fit) {
-      // cluster bundles: among the sizes from S up, the one with the best modelled throughput
-      // B(S) / (fixed per-firing latency + pass time), both ~1 us at 6250 reactions per CTA
+    if (m->opt_state_mode != 1 && S >= s_fit && S >= 2) {
+      // Ensemble throughput = trajectories in flight / time per firing.  Model (measured on B200 with
+      // the candidate-first kernel, profiles/r2_fast_kernel.md): a firing costs ~1.9 us of latency
+      // chain + 0.13 us per 1000 reactions of a CTA, + 1.0 us when the exchange crosses L2.  Clusters
+      // exchange faster but tile the chip worse (7 clusters of 16 = 112 SMs, against 12 L2 bundles of
+      // 12 = 144 SMs): cfg5b runs 3.1e6 trajectory-steps/s as 12 x 12 through L2, 2.3e6 as 7 x 16.
+      // In flight = n_traj / rounds, rounds = ceil(n_traj / bundles).
       double best = 0.0;
-      int best_S = 0;
-      for (int c = S; c <= std::min(rt::kMaxClusterCtas, s_thin); ++c) {
-        const int bc = (int)std::min<u64>(n_traj, (u64)max_active_clusters(m, c));
-        const double thr = bc / (1.0 + (double)pairs_total / c / 3125.0);
-        if (thr > best) { best = thr; best_S = c; }
+      int best_S = S;
+      bool best_cluster = false;
+      const int s_hi = std::min(std::min(s_thin, sms), std::max(S, 2 * rt::kMaxClusterCtas));
+      for (int c = std::max(2, s_fit); c <= s_hi; ++c) {
+        const double t_cta = 1.9 + 0.13 * (2.0 * pairs_total / c / 1000.0);
+        for (int cl = 0; cl < 2; ++cl) {
+          if (cl && (!may_cluster || c > rt::kMaxClusterCtas)) continue;
+          const u64 bundles = cl ? (u64)max_active_clusters(m, c) : (u64)(sms / c);
+          if (bundles == 0) continue;
+          const u64 bb = std::min<u64>(n_traj, bundles);
+          const double in_flight = (double)n_traj / (double)((n_traj + bb - 1) / bb);
+          const double thr = in_flight / (t_cta + (cl ? 0.0 : 1.0));
+          if (thr > best) { best = thr; best_S = c; best_cluster = cl != 0; }
+        }
       }
-      if (best_S) S = best_S;
+      S = best_S;
+      force_l2 = !best_cluster;
     }
   }
   S = std::max(std::min(S, rt::kMaxBundleCtas), 1);
@@ -288,7 +302,7 @@ Plan plan_bundles_for(rt_model *m, u64 n_traj, bool fast) {
   pl.smem = m->opt_state_mode != 1 && smem_state_bytes(pl.pairs_per_cta, fast) <= smem_budget(fast);
   pl.fast = fast && pl.smem;
   pl.cnt_pad = padded_count(pl.pairs_per_cta, pl.fast);
-  if (may_cluster && pl.smem && S >= 2 && S <= rt::kMaxClusterCtas) {
+  if (may_cluster && !force_l2 && pl.smem && S >= 2 && S <= rt::kMaxClusterCtas) {
     B = (int)std::min<u64>(std::max<u64>(n_traj, 1), (u64)max_active_clusters(m, S));
     cluster = B >= 1;
   }
