@@ -206,6 +206,9 @@ int rt_set_rate_exponent(rt_model *m, const double *lambda);
  *                    array: T_out then holds -R_k and P_out zeros).  Same process, different
  *                    rounding: its sample paths match oracle_run_residual, not oracle_run.
  *   "x_replicas"     copies of X per trajectory the CTAs spread their updates over (default 1)
+ *   "pipeline"       1 = candidate-first kernel (rt_fast.cuh) wherever it applies: state in shared
+ *                    memory, "refresh_mode" 0, constant rates, one copy of X (default);
+ *                    0 = always the plain bundle kernel (rt_bundle.cuh).  Same results either way.
  *   "exchange"       0 = a bundle of 2..16 CTAs with on-chip state runs as ONE thread-block cluster
  *                    and reduces its per-firing argmin through distributed shared memory (default),
  *                    1 = always exchange through slots in global memory (L2)
@@ -218,6 +221,7 @@ int rt_set_option(rt_model *m, const char *name, int64_t value);
  *   "ensemble_path"    path taken by the last rt_ensemble call (1 or 2)
  *   "state_in_smem"    1 if the last bundle launch kept (T,P,a) in shared memory
  *   "cluster_exchange" 1 if the last bundle launch ran each bundle as a thread-block cluster
+ *   "pipeline"         1 if the last bundle launch used the candidate-first kernel
  *   "num_sms", "dep_entries", "max_sigma", "hub_species"
  * Unknown name: returns RT_ERR_BAD_ARG and leaves *value alone. */
 int rt_get_info(const rt_model *m, const char *name, int64_t *value);
