@@ -58,20 +58,24 @@ def test_cfg3_scaled_trace(rt, scale, firings, refresh_mode):
                options=[("refresh_mode", refresh_mode)])
 
 
+@pytest.mark.parametrize("pipeline", [1, 0])
 @pytest.mark.parametrize("exchange", [0, 1])
 @pytest.mark.parametrize("ctas", [1, 2, 7, 12, 16, 0])
-def test_cfg3_bundle_shape_invariance(rt, ctas, exchange):
+def test_cfg3_bundle_shape_invariance(rt, ctas, exchange, pipeline):
     """Result must not depend on how many CTAs share the trajectory (determinism contract), nor on
-    how they exchange their partial argmins: as one thread-block cluster through distributed
-    shared memory (exchange 0, bundles of 2..16 CTAs) or through slots in L2 (exchange 1)."""
+    how they exchange their partial argmins -- as one thread-block cluster through distributed
+    shared memory (exchange 0, bundles of 2..16 CTAs) or through slots in L2 (exchange 1) -- nor on
+    the kernel: candidate-first (pipeline 1, rt_fast.cuh) or pass-then-reduce (0, rt_bundle.cuh)."""
     net, x0, par = W.make_config("cfg3", scale=0.02)
     _check_run(rt, net, x0, par["seed"], 3, 1500, math.inf, 1500,
-               options=[("bundle_ctas", ctas), ("exchange", exchange)])
+               options=[("bundle_ctas", ctas), ("exchange", exchange), ("pipeline", pipeline)])
     with rt.Model(net) as m:
         m.set_option("bundle_ctas", ctas)
         m.set_option("exchange", exchange)
+        m.set_option("pipeline", pipeline)
         m.run(x0, par["seed"], 3, 10)
         S = m.info("bundle_ctas")
+        assert m.info("pipeline") == pipeline
         assert m.info("cluster_exchange") == (1 if exchange == 0 and 2 <= S <= 16 else 0)
         if ctas:
             assert S == ctas
@@ -111,9 +115,9 @@ def _hub_network(n_species=40, n_reactions=5000, seed=3):
 @pytest.mark.parametrize("ctas,state_mode,exchange", [(1, 0, 0), (1, 1, 0), (5, 0, 0), (5, 0, 1), (0, 0, 0), (0, 0, 1)])
 def test_hub_species_general_rows_and_staging_overflow(rt, ctas, state_mode, exchange):
     net, x0 = _hub_network()
-    for refresh_mode in (0, 1):
+    for refresh_mode, pipeline in ((0, 1), (0, 0), (1, 1)):
         _check_run(rt, net, x0, 21, 0, 600, math.inf, 600,
-                   options=[("bundle_ctas", ctas), ("state_mode", state_mode),
+                   options=[("bundle_ctas", ctas), ("state_mode", state_mode), ("pipeline", pipeline),
                             ("refresh_mode", refresh_mode), ("exchange", exchange)])
 
 
@@ -230,6 +234,58 @@ def test_exact_ties_go_to_the_lowest_index(rt, ctas, state_mode, formulation):
     opts = [("bundle_ctas", ctas), ("state_mode", state_mode & 1), ("exchange", 1 if state_mode == 2 else 0)]
     _check_tie(rt, 5003, False, formulation, opts)
     _check_tie(rt, 4999, True, formulation, opts)
+
+
+@pytest.mark.parametrize("ctas,exchange", [(1, 0), (3, 0), (3, 1), (16, 0), (0, 1)])
+def test_exact_ties_plain_bundle_kernel(rt, ctas, exchange):
+    """The same tie networks through the pass-then-reduce kernel (pipeline 0) with on-chip state."""
+    opts = [("bundle_ctas", ctas), ("exchange", exchange), ("pipeline", 0)]
+    for formulation in (0, 1):
+        _check_tie(rt, 5003, False, formulation, opts)
+        _check_tie(rt, 4999, True, formulation, opts)
+
+
+def _check_resume_state(rt, net, x0, T0, P0, n, options):
+    M = len(T0)
+    n0 = np.zeros(M, dtype=np.uint64)
+    o = _oracle().run_from(net, x0, 0.0, T0, P0, n0, 9, 1, n, math.inf, n)
+    with rt.Model(net) as m:
+        for name, val in options:
+            m.set_option(name, val)
+        g = m.run_resume(x0, 0.0, T0, P0, n0, 9, 1, n, math.inf, n, want_state=True)
+    np.testing.assert_array_equal(g["trace_mu"], o["trace_mu"])
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["fire_count"], o["fire_count"])
+    np.testing.assert_allclose(g["trace_t"], o["trace_t"], rtol=RTOL_T, atol=0)
+    np.testing.assert_allclose(g["T"], o["T"], rtol=1e-10, atol=1e-12)
+    return g, o
+
+
+@pytest.mark.parametrize("pipeline", [1, 0])
+@pytest.mark.parametrize("ctas,exchange", [(1, 0), (4, 0), (4, 1), (0, 0)])
+def test_near_ties_and_cancellation_defeat_the_filters(rt, ctas, exchange, pipeline):
+    """Adversarial states for the approximate-quotient filters and for the candidate-first kernel's
+    lagged candidates (rt_fast.cuh header).  (a) near-ties: every waiting time within 1e-9 .. 1e-6
+    relative of every other one -- far inside the key tolerance, never equal -- so that no thread
+    can rule anything out and every firing goes through the exact paths.  (b) catastrophic
+    cancellation: internal times ~2^40 with residuals of order 1 (P - T keeps 2^-40 of P: outside
+    the cancellation guard), as after a very long run, mixed with ordinary channels; one rounding
+    of T + a*dt then moves a waiting time by more than the filters' margin, so a candidate kept
+    across a firing without the guard could lose the argmin.  Both against oracle.run_from."""
+    rng = np.random.default_rng(5)
+    M = 4801
+    net, x0, _, _, _ = tie_network(M, coupled=True)
+    a0 = tie_network(M, coupled=True)[3] / 8.0            # a_k(X0), exact (see tie_cases.py)
+    opts = [("bundle_ctas", ctas), ("exchange", exchange), ("pipeline", pipeline)]
+    # (a) dt_k = 8 * (1 + eps_k), eps_k in [1e-9, 1e-6]
+    eps = 10.0 ** rng.uniform(-9, -6, size=M)
+    _check_resume_state(rt, net, x0, np.zeros(M), a0 * 8.0 * (1.0 + eps), 600, opts)
+    # (b) every third channel carries a huge internal time; waiting times spread over a decade
+    big = (np.arange(M) % 3 == 1)
+    T0 = np.where(big, 2.0 ** 40 * (1.0 + rng.uniform(0, 1, size=M)), 0.0)
+    P0 = T0 + a0 * 10.0 ** rng.uniform(-1, 0, size=M)
+    g, o = _check_resume_state(rt, net, x0, T0, P0, 900, opts)
+    assert big[g["trace_mu"]].sum() > 100 and (~big)[g["trace_mu"]].sum() > 100
 
 
 def test_exact_ties_full_recompute_and_thread_kernel(rt):

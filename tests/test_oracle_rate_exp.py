@@ -150,3 +150,27 @@ def test_kurtz_identity_and_clock_invariants():
     assert np.array_equal(x, r["x"]) and (r["x"] >= 0).all()
     assert r["fire_count"].sum() == 1500 and (np.diff(r["trace_t"]) >= 0).all()
     assert (r["T"] <= r["P"] * (1 + 1e-12)).all()
+
+
+def test_common_lambda_is_a_time_change_of_the_constant_rate_run():
+    """Eq.28 with ONE lambda for every channel: int_0^t a_k(s) ds = a_k(X) * s(t) with the same
+    s(t) = (exp(lambda t) - 1) / lambda for all k, so the run is the constant-rate run (same seed,
+    hence same internal firing times P_k) under the time change s -> t(s) = log1p(lambda s) / lambda:
+    same fired sequence, event times t(s_i).  With lambda < 0 internal time saturates at
+    1 / |lambda|: the run fires exactly the constant-rate firings with s_i < 1 / |lambda|, then is
+    ABSORBED.  (lambda is put BETWEEN two firing times: on one, the last argument is -1 +- rounding.)"""
+    net, x0 = W.lotka_volterra(y1=80, y2=60, c1=1.5, c2=0.01, c3=1.0)
+    M = int(net["n_reactions"])
+    base = oracle.run(net, x0, 17, 3, 400, math.inf, 400)
+    s = base["trace_t"]
+    for n_keep, sign in ((150, -1.0), (300, -1.0), (400, +1.0)):
+        if sign < 0:
+            lam = -2.0 / float(s[n_keep - 1] + s[n_keep])           # 1/|lam| between firing n_keep-1 and n_keep
+            o = oracle.run_rate_exp(net, x0, np.full(M, lam), 17, 3, 100000, math.inf, 400)
+            assert o["stop"] == 3 and o["firings"] == n_keep         # ABSORBED
+        else:
+            lam = 0.5 / float(s[-1])
+            o = oracle.run_rate_exp(net, x0, np.full(M, lam), 17, 3, n_keep, math.inf, 400)
+            assert o["firings"] == n_keep
+        np.testing.assert_array_equal(o["trace_mu"][:n_keep], base["trace_mu"][:n_keep])
+        np.testing.assert_allclose(o["trace_t"][:n_keep], np.log1p(lam * s[:n_keep]) / lam, rtol=1e-9)
