@@ -21,6 +21,7 @@ from helpers.direct_method import direct_method
 from helpers.exact_kurtz import exact_path
 from helpers.tie_cases import tie_network, expected_trace
 from helpers.rta_table1 import rta_table1
+from helpers.table3_literal import table3_literal
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 INF = math.inf
@@ -412,6 +413,27 @@ def test_agrees_in_distribution_with_table1_random_time_algorithm(case):
 
 
 # ------------------------------------------------------------------ residual (Table 3) form
+def test_table3_literal_rescale_form_agrees_in_distribution():
+    """PAPER.md Table 3 (:262-272) as printed -- (Delta t_k, p_k), Delta t_k rescaled by p_k/a_k --
+    on a network whose propensities never vanish (where the form is defined: reading G4), against
+    both oracle forms: species marginals at t_end agree (two-sample KS / z-test as elsewhere).
+    Immigration 0 -> S1, autocatalysis S1 -> 2 S1 and S1 -> S1 + S2, catalysed S0 -> S0 + S2 with a
+    conserved catalyst: every a_k > 0 for all time, and three of them change at every firing."""
+    net = W.from_reactions(3, [({}, {1: 1}, 2.0), ({1: 1}, {1: 2}, 0.4), ({1: 1}, {1: 1, 2: 1}, 0.3),
+                               ({0: 1}, {0: 1, 2: 1}, 0.7)])
+    x0, t_end, n_traj = [4, 6, 0], 2.5, 1500
+    xt = table3_literal(net, x0, n_traj, t_end, seed=777)
+    out = oracle.ensemble(net, x0, seed=33, traj_first=0, n_traj=n_traj, t_end=t_end, n_threads=4)
+    res = np.array([oracle.run_residual(net, x0, 34, i, 0, t_end)["x"] for i in range(n_traj)])
+    assert (xt[:, 0] == 4).all() and (out["x"][:, 0] == 4).all()
+    for j in (1, 2):
+        _two_sample(out["x"][:, j].astype(float), xt[:, j].astype(float))
+        _two_sample(res[:, j].astype(float), xt[:, j].astype(float))
+    # closed form for the mean of S1 (linear birth with immigration): E S1(t) = (x0 + c0/c1) e^{c1 t} - c0/c1
+    mean = (6 + 2.0 / 0.4) * math.exp(0.4 * t_end) - 2.0 / 0.4
+    assert abs(xt[:, 1].mean() - mean) < 4.0 * xt[:, 1].std() / math.sqrt(n_traj)
+
+
 def test_residual_form_single_source_closed_form():
     """Table 3: one source channel, a = c constant, so Delta t_i = E_i / c and
     t_n = sum_i fl(E_i / c) with the same draws E(seed, traj, 0, i) as the (T, P) form."""
