@@ -184,7 +184,9 @@ int padded_count(int pairs_per_cta, bool fast) {
   return (2 * pairs_per_cta + batch - 1) / batch * batch;
 }
 size_t smem_state_bytes(int pairs_per_cta, bool fast) {
-  return (size_t)padded_count(pairs_per_cta, fast) * 3 * sizeof(double);
+  size_t slots = (size_t)padded_count(pairs_per_cta, fast);
+  if (fast) slots = slots / stream_threads(true) * (stream_threads(true) + 1);   // padded rows (rt_fast.cuh sidx)
+  return slots * 3 * sizeof(double);
 }
 
 // The bundle kernel for a launch shape (FULL = refresh_mode 1; rate: 0 constant, 1 schedule, 2 exponential).
@@ -249,7 +251,8 @@ Plan plan_bundles_for(rt_model *m, u64 n_traj, bool fast) {
   const int sms = m->num_sms;
   // fewest CTAs whose share of the state still fits in shared memory
   const int batch = rt::kScanBatch * stream_threads(fast);
-  const int pairs_fit = std::max(1, (int)(smem_budget(fast) / (3 * sizeof(double)) / batch * batch / 2));
+  const int pairs_fit = std::max(1, (int)((smem_budget(fast) - (fast ? 64 * 3 * sizeof(double) : 0)) /
+                                          (3 * sizeof(double)) / batch * batch / 2));
   const int s_fit = (pairs_total + pairs_fit - 1) / pairs_fit;
   const int s_thin = std::max(1, (pairs_total + kMinPairsPerCta - 1) / kMinPairsPerCta);
   const bool may_cluster = m->opt_exchange != 1 && m->opt_state_mode != 1;

@@ -73,6 +73,13 @@ struct FastCtx {
   alignas(8) u64 cl_bar[2];
 };
 
+// Shared-memory layout of a CTA's (T, P, a) arrays: reaction li (local index) belongs to stream
+// thread li % NT, slot li / NT, and sits at thread + slot * (NT + 1).  The padded row keeps the
+// slots of ONE thread in different banks, so that a warp re-scanning a stale thread (S3: lane l
+// takes slot l) reads without bank conflicts (with rows of NT they are 32-way: NT is a multiple
+// of 32); the pass itself (lane l = thread l, one slot) is conflict-free either way.
+template <int NT> __device__ __forceinline__ int sidx(int li) { return li + li / NT; }
+
 // Integer key of the approximate quotient of one reaction; clears guard_ok when the lagged
 // candidate argument does not cover it (see the header).
 __device__ __forceinline__ int q_key(double pk, double t, double a, bool &guard_ok) {
@@ -93,15 +100,16 @@ __device__ __forceinline__ int pass_and_pick(int tid, int cnt_pad, double *__res
   int m1 = 0x7fffffff, m2 = 0x7fffffff, s1 = 0;
   bool guard_ok = true;
   int slot = 0;
-  for (int i = tid; i < cnt_pad; i += U * NT, slot += U) {
+  constexpr int R = NT + 1;                            // padded row (see sidx)
+  for (int i = tid; i < cnt_pad; i += U * R, slot += U) {
     double a[U], t[U], pk[U];
 #pragma unroll
-    for (int u = 0; u < U; ++u) { a[u] = sA[i + u * NT]; t[u] = sT[i + u * NT]; pk[u] = sP[i + u * NT]; }
+    for (int u = 0; u < U; ++u) { a[u] = sA[i + u * R]; t[u] = sT[i + u * R]; pk[u] = sP[i + u * R]; }
 #pragma unroll
     for (int u = 0; u < U; ++u)
       if (!((done >> (slot + u)) & 1ull)) {
         t[u] = __dadd_rn(t[u], __dmul_rn(a[u], dprev));
-        sT[i + u * NT] = t[u];
+        sT[i + u * R] = t[u];
       }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
@@ -122,13 +130,14 @@ __device__ __forceinline__ void pass_advance(int tid, int cnt_pad, double *__res
                                              const double *__restrict__ sA, double dprev, u64 done) {
   constexpr int U = kScanBatch;
   int slot = 0;
-  for (int i = tid; i < cnt_pad; i += U * NT, slot += U) {
+  constexpr int R = NT + 1;
+  for (int i = tid; i < cnt_pad; i += U * R, slot += U) {
     double a[U], t[U];
 #pragma unroll
-    for (int u = 0; u < U; ++u) { a[u] = sA[i + u * NT]; t[u] = sT[i + u * NT]; }
+    for (int u = 0; u < U; ++u) { a[u] = sA[i + u * R]; t[u] = sT[i + u * R]; }
 #pragma unroll
     for (int u = 0; u < U; ++u)
-      if (!((done >> (slot + u)) & 1ull)) sT[i + u * NT] = __dadd_rn(t[u], __dmul_rn(a[u], dprev));
+      if (!((done >> (slot + u)) & 1ull)) sT[i + u * R] = __dadd_rn(t[u], __dmul_rn(a[u], dprev));
   }
 }
 
@@ -172,9 +181,10 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
   const int k0 = 2 * q0, k1 = 2 * q1;
   const int cnt_pad = p.cnt_pad;
   const int nslot = cnt_pad / NT;                     // slots per stream thread (<= 64)
+  const int cnt_row = nslot * (NT + 1);               // array length with padded rows (see sidx)
   double *sT = reinterpret_cast<double *>(dyn_smem);
-  double *sP = sT + cnt_pad;
-  double *sA = sP + cnt_pad;
+  double *sP = sT + cnt_row;
+  double *sA = sP + cnt_row;
 
   uint32_t gen = 0;
   if (tid == 0) {
@@ -211,14 +221,15 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           t_init = resid ? -e0 : 0.0; p_init = resid ? 0.0 : e0;
         }
       } else if (resid) { t_init = -1.0; p_init = 0.0; }
-      sT[k - k0] = t_init; sP[k - k0] = p_init; sA[k - k0] = a0;
+      const int si = sidx<NT>(k - k0);
+      sT[si] = t_init; sP[si] = p_init; sA[si] = a0;
       if (k < k1) nfire[k] = n_init;
     }
     __syncthreads();
     // candidates of the first firing (nothing to advance)
     int cand_slot = -1;
     if (is_stream) {
-      cand_slot = pass_and_pick<NT>(tid, cnt_pad, sT, sP, sA, 0.0, ~0ull, ctx.any_odd != 0);
+      cand_slot = pass_and_pick<NT>(tid, cnt_row, sT, sP, sA, 0.0, ~0ull, ctx.any_odd != 0);
       mybest_k[tid] = cand_slot >= 0 ? k0 + tid + cand_slot * NT : -3;
       dirty[tid] = cand_slot < 0;
     }
@@ -247,19 +258,19 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         // ===== S1: advance and divide the candidate; also advance the reaction that fired
         u64 mask = 0;
         if (cand_slot >= 0) {
-          const int i = tid + cand_slot * NT;
+          const int i = tid + cand_slot * (NT + 1);
           const double a = sA[i];
           const double tn = __dadd_rn(sT[i], __dmul_rn(a, dprev));
           sT[i] = tn;
           best.dt = waiting_time(sP[i], tn, a);
-          best.k = k0 + i;
+          best.k = k0 + tid + cand_slot * NT;
           mask = 1ull << cand_slot;
         }
         if (mu_prev >= k0 && mu_prev < k1 && (mu_prev - k0) % NT == tid) {
           // a-7: this thread owns the reaction that fired: new internal firing time (Eq.26), as a rule
           // precomputed when the reaction became the thread's candidate (S5)
-          const int i = mu_prev - k0;
-          const u64 bit = 1ull << (i / NT);
+          const int i = sidx<NT>(mu_prev - k0);
+          const u64 bit = 1ull << ((mu_prev - k0) / NT);
           if (spec_k != mu_prev) {
             spec_n = nfire[mu_prev] + 1u;
             const double e_new = exp_draw(p.seed, traj, (uint32_t)mu_prev, spec_n);
@@ -398,7 +409,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           for (int i = tid; i < n; i += NT) {
             const int k = lk[i];
             const double a_new = la[i];
-            const int li = k - k0, o = li % NT, slot = li / NT;
+            const int o = (k - k0) % NT, slot = (k - k0) / NT, li = o + slot * (NT + 1);   // li: index in shared memory
             if (!mask_claim(refm, o, slot)) continue;         // (a reaction reading two changed species is listed twice)
             if (mask_claim(advm, o, slot))                    // T_k += a_k dt with the OLD a_k, once
               sT[li] = __dadd_rn(sT[li], __dmul_rn(sA[li], dprev));
@@ -448,7 +459,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           const u64 m = mask_load(advm, th);
           const int j0 = lane, j1 = lane + 32;
           const bool h0 = j0 < nslot, h1 = j1 < nslot;
-          const int i0 = th + j0 * NT, i1 = th + j1 * NT;
+          const int i0 = th + j0 * (NT + 1), i1 = th + j1 * (NT + 1);     // (shared memory)
+          const int kk0 = k0 + th + j0 * NT, kk1 = kk0 + 32 * NT;        // (reactions)
           double a0 = 0.0, p0 = 1.0, t0 = 0.0, a1 = 0.0, p1 = 1.0, t1 = 0.0;
           if (h0) { a0 = sA[i0]; p0 = sP[i0]; t0 = sT[i0]; }
           if (h1) { a1 = sA[i1]; p1 = sP[i1]; t1 = sT[i1]; }
@@ -461,10 +473,10 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           const bool trust = ctx.any_odd == 0 && sm1 >= ((1023 - 100) << 20) && sm1 <= ((1023 + 100) << 20);
           const int lim = trust ? sm1 + kQTolUnits : 0x7fffffff;
           Cand c = none;
-          if (h0 && sq0 <= lim) { c.dt = waiting_time(p0, t0, a0); c.k = k0 + i0; }
+          if (h0 && sq0 <= lim) { c.dt = waiting_time(p0, t0, a0); c.k = kk0; }
           if (h1 && sq1 <= lim) {
             const double d = waiting_time(p1, t1, a1);
-            if (cand_less(d, k0 + i1, c)) { c.dt = d; c.k = k0 + i1; }
+            if (cand_less(d, kk1, c)) { c.dt = d; c.k = kk1; }
           }
           c = warp_lexmin(c);
           __syncwarp();
@@ -505,11 +517,11 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         newcand[tid] = -1;
         pick = pick || (((unsigned)fired + (unsigned)warp) % kRepickPeriod == 0u);
         if (__any_sync(0xffffffffu, pick)) {
-          cand_slot = pass_and_pick<NT>(tid, cnt_pad, sT, sP, sA, dprev, mask_load(advm, tid), ctx.any_odd != 0);
+          cand_slot = pass_and_pick<NT>(tid, cnt_row, sT, sP, sA, dprev, mask_load(advm, tid), ctx.any_odd != 0);
           mybest_k[tid] = cand_slot >= 0 ? k0 + tid + cand_slot * NT : -3;
           if (cand_slot < 0) dirty[tid] = 1;
         } else {
-          pass_advance<NT>(tid, cnt_pad, sT, sA, dprev, mask_load(advm, tid));
+          pass_advance<NT>(tid, cnt_row, sT, sA, dprev, mask_load(advm, tid));
         }
         repick[tid] = 0;
         mask_store(advm, tid, 0);
@@ -520,7 +532,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
           spec_k = mybest_k[tid];
           spec_n = nfire[spec_k] + 1u;
           const double e_new = exp_draw(p.seed, traj, (uint32_t)spec_k, spec_n);
-          spec_P = resid ? -e_new : __dadd_rn(sP[spec_k - k0], e_new);
+          spec_P = resid ? -e_new : __dadd_rn(sP[sidx<NT>(spec_k - k0)], e_new);
         }
       } else if (is_xw) {
         if (!finishing) named_sync<NT + 32>(kBarParts);
@@ -658,7 +670,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
     if (!bundle_barrier<BLOCK, CLUSTER>(exch, p.S, r, gen, p.err)) return;
     if (!CLUSTER) gen += 1u;
     for (int k = k0 + tid; k < k1; k += BLOCK) {
-      __stcg(T + k, sT[k - k0]); __stcg(P + k, sP[k - k0]); __stcg(A + k, sA[k - k0]);
+      const int si = sidx<NT>(k - k0);
+      __stcg(T + k, sT[si]); __stcg(P + k, sP[si]); __stcg(A + k, sA[si]);
     }
     if (p.x_out)
       for (int j = r * BLOCK + tid; j < N; j += p.S * BLOCK)
