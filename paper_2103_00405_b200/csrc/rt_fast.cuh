@@ -14,29 +14,34 @@
 //       their warp sharing the work;
 //   S4  block argmin -> the exchange warp posts this CTA's partial;
 //   S5  WHILE the exchange is in flight the stream warps run the pass: T_k += a_k dt for every
-//       reaction not advanced in S1..S3 (per-thread bit masks), approximate quotients, and the
-//       choice of the thread's candidate for the NEXT firing.
+//       reaction not advanced in S1..S3 (per-thread bit masks).  A thread keeps its candidate
+//       across firings; its warp re-derives the candidates from approximate quotients when one
+//       is void or doubtful, and at least every kRepickPeriod firings.
 // Every T_k still receives every increment a_k dt_n, one rounded multiply and one rounded add per
 // firing, in firing order: results are bit-identical to dividing everything every firing.
 //
-// Why a candidate chosen one firing early is still the thread's exact argmin:
-// the pass looks at the HIGH WORD of q~_k = (P_k - T_k) * rcp.approx(a_k) as an integer key
-// (positive doubles order like integers).  Key error: rcp.approx.ftz.f64 2^-19.9 relative
+// Why a candidate chosen earlier is still the thread's exact argmin: the pass looks
+// at the HIGH WORD of q~_k = (P_k - T_k) * rcp.approx(a_k) as an integer key (positive doubles
+// order like integers).  Key error: rcp.approx.ftz.f64 2^-19.94 relative
 // (tests/test_gpu_kernel_facts.py), truncation < 1 unit; a unit is 2^-20..2^-21 relative, so a key
 // is within 3.5 units of the exact quotient's.  One more firing moves every exact quotient of the
-// thread by the same dt, except for the rounding of T_k + a_k dt, which is at most
-// 2^-51 max(|T_k|, |P_k|) / a_k: the pass checks that P_k - T_k keeps at least 2^-31 of
-// max(|P_k|, |T_k|) (kGuardShift; integer test on high words), which bounds that error by 2 units.
-// A thread whose second-smallest key exceeds the smallest by more than kQTolUnits = 32 > 2 (3.5 + 2)
-// therefore has a unique exact argmin after the next firing too; any other thread has no candidate
-// and is re-scanned exactly (S3), as are all threads when some a_k of the CTA is outside the range
-// where the rcp bound is established (any_odd).
+// thread by the same dt, except for the rounding of T_k + a_k dt, at most
+// 2^-52 (|T_k| + a_k dt) / a_k: the pass checks that P_k - T_k keeps at least 2^-31 of
+// max(|P_k|, |T_k|) (kGuardShift; integer test on high words; a_k = 0 exempt), which bounds that
+// drift by one unit per reaction per firing.  A thread whose second-smallest key exceeds the
+// smallest by more than kQTolUnits = 64 > 2 * 3.5 + 2 * kRepickPeriod therefore keeps a unique
+// exact argmin for kRepickPeriod = 24 firings; a refreshed reaction is compared exactly (S2: it
+// must stay 2^-13 clear of the candidate, or clearly below it and take over, else the thread
+// re-picks); any thread without such a margin has no candidate and is re-scanned exactly every
+// firing (S3), as are all threads when some a_k of the CTA is outside the range where the rcp
+// bound is established (any_odd).
 //
-// Warps: NT / 32 stream warps, one exchange warp (reduces the warp partials, posts, precomputes the
-// redraw of this CTA's candidate while the exchange is in flight, gathers), one walker warp (X
+// Warps: NT / 32 stream warps; one exchange warp (reduces the warp partials, posts, gathers,
+// publishes the winner, prefetches the CTA candidate's walk data into L2); one walker warp (X
 // update, staged refreshes; while the others work it pre-walks the exchange's runner-up AND
 // computes that reaction's refreshes speculatively from X as it will be, so that a correct guess
-// -- 94..99 % of the firings -- costs no memory round trip at all).
+// -- 94..99 % of the firings -- costs no memory round trip at all).  The redraw of P_mu (Philox +
+// log) is precomputed by each stream thread for its own candidate and installed by the owner in S1.
 #pragma once
 #include "rt_bundle.cuh"
 
