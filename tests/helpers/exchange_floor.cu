@@ -12,6 +12,8 @@
 //           polled line has ONE reader and is written by one CTA per slot
 //   l2near  every slot exists in 4 copies 8 MiB apart; a CTA polls the copy it reads fastest
 //           (l2copies: the same 4 stores, but everybody polls copy 0)
+//   l2die   148 CTAs in two groups by SM id half (l2parity: by SM id parity, a control), each group
+//           gathering on its own slots
 //   dsmem   the C CTAs of one thread-block cluster post into every peer's shared memory with
 //           st.async (remote store + complete_tx on the peer's mbarrier), each waits on its own
 //           mbarrier: no global memory on the path
@@ -178,6 +180,35 @@ __global__ void __launch_bounds__(32, 1) k_l2near(u64 *exch, int S, int rounds, 
   if (lane == 0) out[r] = val;
 }
 
+
+// ---- l2die: the CTAs are split into two groups by SM id (< 74 or not: the two dies, if SM ids are
+// laid out that way) and each group all-gathers on its own slots: does locality lower the floor?
+// GROUPING 0: by SM id half; 1: by SM id parity (a control: same group sizes, no locality).
+template <int GROUPING>
+__global__ void __launch_bounds__(32, 1) k_l2die(u64 *exch, unsigned *counters, int rounds, u64 *out) {
+  const int lane = threadIdx.x;
+  unsigned smid;
+  asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+  const int grp = GROUPING == 0 ? (smid >= 74u ? 1 : 0) : (int)(smid & 1u);
+  __shared__ int s_rank, s_size;
+  if (lane == 0) s_rank = (int)atomicAdd(&counters[grp], 1u);
+  __syncwarp();
+  cooperative_groups::this_grid().sync();
+  if (lane == 0) s_size = (int)counters[grp];
+  __syncwarp();
+  const int r = s_rank, S = s_size;
+  u64 *base = exch + (size_t)grp * 2 * 256 * kSlotStride;
+  u64 val = (u64)blockIdx.x + 1;
+  for (int g = 0; g < rounds; ++g) {
+    const u64 tag = (u64)g + 1;
+    u64 *buf = base + (size_t)(g & 1) * 256 * kSlotStride;
+    if (lane == 0) st_relaxed_v2(buf + (size_t)kSlotStride * r, val, tag);
+    const u64 m = poll_min(buf, S, lane, tag);
+    val = m + (u64)blockIdx.x + 1;
+  }
+  if (lane == 0) out[blockIdx.x] = val + (u64)S;
+}
+
 // ---- MODE 0 dsmem, 1 hybrid (all poll), 2 hyblead (leaders poll, DSMEM broadcast), 3 hybpush
 template <int MODE>
 __global__ void __launch_bounds__(32, 1) k_cluster(u64 *exch, int C, int n_clusters, int rounds, u64 *out) {
@@ -329,6 +360,30 @@ int main() {
       }
       printf("%s,%d,1,%d,%.3f\n", cal ? "l2near" : "l2copies", S, S, best * 1e3 / rounds);
     }
+  for (int grouping = 0; grouping < 2; ++grouping) {
+    unsigned *counters;
+    CK(cudaMalloc(&counters, 8));
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(148); cfg.blockDim = dim3(32); cfg.dynamicSmemBytes = 0;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeCooperative; at[0].val.cooperative = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    void *args[] = {&exch, &counters, &rounds, &out};
+    float best = 1e30f;
+    for (int rep = 0; rep < 3; ++rep) {
+      CK(cudaMemset(exch, 0, exch_bytes));
+      CK(cudaMemset(counters, 0, 8));
+      cudaEvent_t e0, e1;
+      CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+      CK(cudaEventRecord(e0));
+      CK(cudaLaunchKernelExC(&cfg, grouping ? (const void *)k_l2die<1> : (const void *)k_l2die<0>, args));
+      CK(cudaEventRecord(e1));
+      CK(cudaDeviceSynchronize());
+      float ms; CK(cudaEventElapsedTime(&ms, e0, e1));
+      if (ms < best) best = ms;
+    }
+    printf("%s,148,1,2,%.3f\n", grouping ? "l2parity" : "l2die", best * 1e3 / rounds);
+  }
   for (int C : {2, 4, 6, 8, 16}) {
     cudaLaunchConfig_t cfg = {};
     cfg.blockDim = dim3(32); cfg.dynamicSmemBytes = dyn;
