@@ -383,7 +383,8 @@ int launch_bundles(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
     at[0].val.cooperative = 1;
   }
   cfg.attrs = at; cfg.numAttrs = 1;
-  if (pl.smem && m->l2_limit_set) {             // (give the set-aside part of L2 back to everybody)
+  if (m->l2_limit_set && (pl.smem || !m->opt_l2_persist)) {   // (give the set-aside part of L2 back to everybody;
+                                                               //  lines made persisting earlier would stay so)
     cudaCtxResetPersistingL2Cache();
     cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, 0);
     cudaGetLastError();
