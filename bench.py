@@ -332,7 +332,7 @@ def measure(rt, torch, dist, args, workload, steps, warmup, rank, world, local, 
             ginstr = ips * fired_local / kernel_s / 1e9 if ips else None
             out["roofline"] = {"bound": "alu", "achieved": ginstr, "peak": ALU_PEAK_GINSTR,
                                "unit": "Ginstr/s", "frac": ginstr / ALU_PEAK_GINSTR if ginstr else None,
-                               "traffic": None, "kernel": "rt_thread_kernel",
+                               "traffic": None, "kernel": "rt_tiny_kernel" if model.info("tiny_kernel") else "rt_thread_kernel",
                                "peak_source": "148 SMs x 4 schedulers x 32 lanes x 1.965 GHz (DESIGN.md 7)",
                                "thread_instructions_per_step": ips, "thread_instructions_source": src}
         else:

@@ -206,6 +206,9 @@ int rt_set_rate_exponent(rt_model *m, const double *lambda);
  *                    array: T_out then holds -R_k and P_out zeros).  Same process, different
  *                    rounding: its sample paths match oracle_run_residual, not oracle_run.
  *   "x_replicas"     copies of X per trajectory the CTAs spread their updates over (default 1)
+ *   "tiny_kernel"    one-thread-per-trajectory path: 1 = networks of at most 4 reactions (<= 2 reactants
+ *                    each) over at most 4 species use the register-resident kernel (default),
+ *                    0 = always the general shared-memory kernel.  Same results either way.
  *   "l2_persist"     state streamed from global memory only: 1 = keep T (read and written every
  *                    firing) as persisting lines in L2 through an access-policy window on the launch
  *                    (default; the first such launch raises the device's persisting-L2 limit to its
@@ -226,6 +229,7 @@ int rt_set_option(rt_model *m, const char *name, int64_t value);
  *   "state_in_smem"    1 if the last bundle launch kept (T,P,a) in shared memory
  *   "cluster_exchange" 1 if the last bundle launch ran each bundle as a thread-block cluster
  *   "pipeline"         1 if the last bundle launch used the candidate-first kernel
+ *   "tiny_kernel"      1 if the last one-thread-per-trajectory launch used the register-resident kernel
  *   "l2_persist"       the "l2_persist" option in effect (0 if the device has no persisting L2)
  *   "num_sms", "dep_entries", "max_sigma", "hub_species"
  * Unknown name: returns RT_ERR_BAD_ARG and leaves *value alone. */

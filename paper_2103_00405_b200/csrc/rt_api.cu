@@ -93,7 +93,10 @@ struct rt_model {
   DevBuf d_x0, d_xout, d_res, d_trace_mu, d_trace_t, d_T0, d_P0, d_n0;
   // options
   int refresh_mode = 0, opt_bundle_ctas = 0, opt_ensemble_path = 0, opt_state_mode = 0, opt_x_replicas = 0, opt_prefetch = 7, opt_formulation = 0;
-  int opt_exchange = 0, opt_pipeline = 1, opt_l2_persist = 1;
+  int opt_exchange = 0, opt_pipeline = 1, opt_l2_persist = 1, opt_tiny = 1;
+  rt::TinyNet tiny{};        // dense copy of a network small enough for rt_tiny_kernel
+  bool tiny_ok = false;
+  int last_tiny = 0;
   size_t l2_persist_max = 0, l2_window_max = 0;   // device limits for persisting L2 lines / window size
   bool l2_limit_set = false;
   int last_fast = 0;
@@ -447,6 +450,24 @@ int launch_threads(rt_model *m, const long long *x0_dev, u64 seed, u64 traj_firs
   p.net = m->net; p.nnz_r = m->nnz_r; p.nnz_v = m->nnz_v;
   p.x0 = x0_dev; p.seed = seed; p.traj_first = traj_first; p.n_traj = n_traj;
   p.max_firings = max_firings; p.t_end = t_end; p.x_out = x_out_dev; p.res = res_dev;
+  m->last_tiny = 0;
+  if (m->tiny_ok && m->opt_tiny) {
+    rt::TinyParams q{};
+    q.net = m->tiny; q.net.xmax = m->net.xmax;
+    q.x0 = x0_dev; q.seed = seed; q.traj_first = traj_first; q.n_traj = n_traj;
+    q.max_firings = max_firings; q.t_end = t_end; q.x_out = x_out_dev; q.res = res_dev;
+    q.T0 = start.T0; q.P0 = start.P0; q.n0 = start.n0; q.t0 = start.t0;
+    q.T_out = T_out; q.P_out = P_out; q.n_out = n_out;
+    if (n_traj >= (u64)m->num_sms * 2048)
+      rt::rt_tiny_kernel<128><<<(unsigned)((n_traj + 127) / 128), 128, 0, st>>>(q);
+    else
+      rt::rt_tiny_kernel<32><<<(unsigned)((n_traj + 31) / 32), 32, 0, st>>>(q);
+    CU_TRY(cudaGetLastError());
+    m->kernel_launches += 1;
+    m->last_path = 1;
+    m->last_tiny = 1;
+    return RT_OK;
+  }
   // Smallest CTA that still fills the chip: more CTAs -> finer balance over the 148 SMs.
   const size_t s32 = rt::thread_kernel_smem(m->net.M, m->net.N, m->nnz_r, m->nnz_v, 32);
   const size_t s128 = rt::thread_kernel_smem(m->net.M, m->net.N, m->nnz_r, m->nnz_v, 128);
@@ -514,6 +535,22 @@ int rt_create(const rt_network *net, int device, rt_model **out) {
       sv(net->stoich_v, net->stoich_v + nv);
   std::vector<double> rate(net->rate, net->rate + M);
   for (double &c : rate) c += 0.0;     // -0.0 -> +0.0: a_k is then never -0.0 (same results: a_k = 0 either way)
+  // ---- the smallest networks also get a dense by-value table for the register-resident kernel
+  if (M <= rt::kTinyM && N <= rt::kTinyN) {
+    bool ok = true;
+    rt::TinyNet &tn = m->tiny;
+    tn.M = M; tn.N = N;
+    for (int k = 0; k < rt::kTinyM; ++k) {
+      tn.rate[k] = k < M ? rate[k] : 0.0;
+      for (int e = 0; e < 2; ++e) { tn.r_j[k][e] = -1; tn.r_s[k][e] = 1; }
+      for (int j = 0; j < rt::kTinyN; ++j) tn.v[k][j] = 0;
+      if (k >= M) continue;
+      if (rp[k + 1] - rp[k] > 2) { ok = false; break; }
+      for (uint32_t e = rp[k]; e < rp[k + 1]; ++e) { tn.r_j[k][e - rp[k]] = rs[e]; tn.r_s[k][e - rp[k]] = rg[e]; }
+      for (uint32_t e = sp[k]; e < sp[k + 1]; ++e) tn.v[k][ss[e]] = sv[e];
+    }
+    m->tiny_ok = ok;
+  }
   // ---- dependency graph, two-hop: stoich row of mu -> species -> reactions that
   // have the species as a reactant.  Entries of one species ascend in k (counting sort over the
   // reactant CSR, which is ordered by reaction) and carry what a refresh needs.
@@ -837,6 +874,9 @@ int rt_set_option(rt_model *m, const char *name, int64_t value) {
   } else if (!strcmp(name, "state_mode")) {
     if (value < 0 || value > 1) return RT_ERR_BAD_ARG;
     m->opt_state_mode = (int)value;
+  } else if (!strcmp(name, "tiny_kernel")) {
+    if (value < 0 || value > 1) return RT_ERR_BAD_ARG;
+    m->opt_tiny = (int)value;
   } else if (!strcmp(name, "l2_persist")) {
     if (value < 0 || value > 2) return RT_ERR_BAD_ARG;
     m->opt_l2_persist = (int)value;
@@ -865,6 +905,7 @@ int rt_get_info(const rt_model *m, const char *name, int64_t *value) {
   else if (!strcmp(name, "state_in_smem")) *value = m->last_state_smem;
   else if (!strcmp(name, "cluster_exchange")) *value = m->last_cluster;
   else if (!strcmp(name, "pipeline")) *value = m->last_fast;
+  else if (!strcmp(name, "tiny_kernel")) *value = m->last_tiny;
   else if (!strcmp(name, "l2_persist")) *value = (m->opt_l2_persist && m->l2_persist_max > 0 && m->l2_window_max > 0) ? m->opt_l2_persist : 0;
   else if (!strcmp(name, "hub_species")) *value = (int64_t)m->n_big;
   else return RT_ERR_BAD_ARG;

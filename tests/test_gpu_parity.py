@@ -470,6 +470,62 @@ def test_ensemble_thread_path_matches_oracle(rt):
     np.testing.assert_allclose(g["t"], o["t"], rtol=RTOL_T)
 
 
+@pytest.mark.parametrize("tiny", [1, 0])
+def test_tiny_networks_register_and_shared_memory_thread_kernels(rt, tiny):
+    """One thread per trajectory, both kernels: rt_tiny_kernel (state in registers: at most 4
+    reactions of at most 2 reactants over at most 4 species) and the general rt_thread_kernel give
+    the oracle's rows -- stops by t_end, max_firings, absorption and count overflow, sigma = 2 and
+    sigma = 3 reactants, a reaction without reactants, checkpointed single trajectories."""
+    cases = []
+    net, x0, par = W.make_config("cfg2")
+    cases.append((net, x0, par["seed"], 33, 3000, 0.2))
+    net, x0, par = W.make_config("cfg1")
+    cases.append((net, x0, par["seed"], 40, 0, 30.0))
+    # dimerisation 2A <-> B, trimer 3A -> C, source 0 -> A, decay C -> 0 (4 reactions, 3 species)
+    net = W.from_reactions(3, [({0: 2}, {1: 1}, 0.02), ({1: 1}, {0: 2}, 1.0), ({0: 3}, {2: 1}, 1e-4),
+                               ({}, {0: 1}, 5.0)])
+    cases.append((net, np.array([60, 5, 0]), 7, 50, 500, math.inf))
+    # pure death: absorbed
+    net = W.from_reactions(2, [({0: 1}, {1: 1}, 1.0), ({1: 1}, {}, 2.0)])
+    cases.append((net, np.array([30, 0]), 8, 25, 0, 1e9))
+    for net, x0, seed, n, mf, t_end in cases:
+        o = _oracle().ensemble(net, x0, seed, 2, n, mf, t_end)
+        with rt.Model(net) as m:
+            m.set_option("tiny_kernel", tiny)
+            m.set_option("ensemble_path", 1)
+            g = m.ensemble(x0, seed, 2, n, mf, t_end)
+            assert m.info("ensemble_path") == 1 and m.info("tiny_kernel") == tiny
+        np.testing.assert_array_equal(g["x"], o["x"])
+        np.testing.assert_array_equal(g["firings"], o["firings"])
+        np.testing.assert_array_equal(g["stop"], o["stop"])
+        np.testing.assert_allclose(g["t"], o["t"], rtol=RTOL_T)
+    # checkpoint / resume of one trajectory through the thread path
+    net, x0, par = W.make_config("cfg2")
+    with rt.Model(net) as m:
+        m.set_option("tiny_kernel", tiny)
+        m.set_option("ensemble_path", 1)
+        a = m.run(x0, 3, 9, 700, math.inf, want_state=True)
+        b1 = m.run(x0, 3, 9, 300, math.inf, want_state=True)
+        b2 = m.run_resume(b1["x"], b1["t"], b1["T"], b1["P"], b1["fire_count"], 3, 9, 400, math.inf, want_state=True)
+        assert m.info("tiny_kernel") == tiny
+    o = _oracle().run(net, x0, 3, 9, 700, math.inf)
+    np.testing.assert_array_equal(a["x"], o["x"])
+    np.testing.assert_array_equal(b2["x"], a["x"])
+    assert b2["t"] == a["t"]
+    np.testing.assert_array_equal(b2["P"], a["P"])
+    np.testing.assert_array_equal(b2["T"], a["T"])
+    # count overflow on the thread path: the offending update is not applied (DESIGN.md 2)
+    net = W.from_reactions(1, [({}, {0: 1}, 1.0)])
+    xmax = 2**31 - 1
+    with rt.Model(net) as m:
+        m.set_option("tiny_kernel", tiny)
+        m.set_option("ensemble_path", 1)
+        g = m.ensemble(np.array([xmax - 2]), 1, 0, 3, 10, math.inf, check=False)
+    assert g["code"] == rt.RT_ERR_OVERFLOW
+    np.testing.assert_array_equal(g["x"][:, 0], [xmax] * 3)
+    np.testing.assert_array_equal(g["firings"], [3] * 3)
+
+
 def test_ensemble_bundle_path_matches_run_and_oracle(rt):
     """cfg5b shape (several trajectories of one mid-size network): ensemble row i == rt_run(i)
     == oracle trajectory i; thread path and bundle path agree on a tiny network."""
