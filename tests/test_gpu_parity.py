@@ -739,6 +739,33 @@ def test_time_dependent_rates_revive_an_absorbed_state(rt):
     _check_sched(rt, net, x0, 21, 0, 500, math.inf, 500, [0.0, b1, 2 * b1], [0.0, 1.0, 2.5], None)
 
 
+def test_options_are_validated_and_reported(rt):
+    """Every tuning knob of rt.h: out-of-range values and unknown names are refused, accepted values
+    show up in rt_get_info after a launch, and none of them changes a result."""
+    net, x0, par = W.make_config("cfg3", scale=0.02)
+    ranges = {"refresh_mode": (0, 1), "bundle_ctas": (0, 1024), "ensemble_path": (0, 2), "formulation": (0, 1),
+              "prefetch": (0, 7), "x_replicas": (0, 64), "state_mode": (0, 1), "exchange": (0, 1),
+              "pipeline": (0, 1), "l2_persist": (0, 2), "tiny_kernel": (0, 1)}
+    with rt.Model(net) as m:
+        for name, (lo, hi) in ranges.items():
+            for bad in (lo - 1, hi + 1):
+                assert rt.rt_set_option(m.handle, name, bad) == rt.RT_ERR_BAD_ARG, (name, bad)
+            assert rt.rt_set_option(m.handle, name, lo) == rt.RT_OK
+        assert rt.rt_set_option(m.handle, "no_such_option", 0) == rt.RT_ERR_BAD_ARG
+        with pytest.raises(rt.RtError):
+            m.info("no_such_info")
+        base = m.run(x0, 3, 0, 400, math.inf, 400)
+        assert m.info("pipeline") == 0 and m.info("cluster_exchange") == 1 and m.info("state_in_smem") == 1
+        for name, val in (("pipeline", 1), ("exchange", 1), ("prefetch", 0), ("prefetch", 7), ("x_replicas", 2),
+                          ("state_mode", 1), ("l2_persist", 0), ("l2_persist", 1), ("bundle_ctas", 3)):
+            m.set_option(name, val)
+            g = m.run(x0, 3, 0, 400, math.inf, 400)
+            np.testing.assert_array_equal(g["trace_mu"], base["trace_mu"])
+            np.testing.assert_array_equal(g["trace_t"], base["trace_t"])
+            np.testing.assert_array_equal(g["x"], base["x"])
+        assert m.info("state_in_smem") == 0 and m.info("bundle_ctas") == 3 and m.info("l2_persist") in (0, 1)
+
+
 def test_rate_schedule_validation_and_unsupported_combinations(rt):
     net, x0 = W.lotka_volterra()
     with rt.Model(net) as m:
