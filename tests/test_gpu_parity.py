@@ -739,6 +739,30 @@ def test_time_dependent_rates_revive_an_absorbed_state(rt):
     _check_sched(rt, net, x0, 21, 0, 500, math.inf, 500, [0.0, b1, 2 * b1], [0.0, 1.0, 2.5], None)
 
 
+@pytest.mark.parametrize("pipeline,exchange", [(1, 0), (1, 1), (0, 0)])
+def test_ensemble_to_t_end_on_the_bundle_path(rt, pipeline, exchange):
+    """Trajectories of a mid-size network that stop at t_end after DIFFERENT numbers of firings,
+    more trajectories than bundles (the bundles pick up their next trajectory at different times):
+    every row against the oracle, stop reason and clock included."""
+    net, x0, par = W.make_config("cfg3", scale=0.02)
+    o1 = _oracle().run(net, x0, 11, 0, 600, math.inf, 600)
+    t_end = float(o1["trace_t"][450])
+    n = 23
+    o = _oracle().ensemble(net, x0, 11, 0, n, 0, t_end)
+    assert len(set(o["firings"].tolist())) > 5
+    with rt.Model(net) as m:
+        m.set_option("ensemble_path", 2)
+        m.set_option("pipeline", pipeline)
+        m.set_option("exchange", exchange)
+        m.set_option("bundle_ctas", 4)
+        g = m.ensemble(x0, 11, 0, n, 0, t_end)
+        assert m.info("pipeline") == pipeline and m.info("bundles") >= 2
+    np.testing.assert_array_equal(g["x"], o["x"])
+    np.testing.assert_array_equal(g["firings"], o["firings"])
+    np.testing.assert_array_equal(g["stop"], o["stop"])
+    assert (g["stop"] == rt.RT_STOP_T_END).all() and (g["t"] == t_end).all()
+
+
 def test_options_are_validated_and_reported(rt):
     """Every tuning knob of rt.h: out-of-range values and unknown names are refused, accepted values
     show up in rt_get_info after a launch, and none of them changes a result."""
