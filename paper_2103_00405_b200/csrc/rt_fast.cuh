@@ -415,17 +415,23 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
             const int k = lk[i];
             const double a_new = la[i];
             const int o = (k - k0) % NT, slot = (k - k0) / NT, li = o + slot * (NT + 1);   // li: index in shared memory
+            const int ob = mybest_k[o];
+            const double t_old = sT[li], a_old = sA[li], pk = sP[li];
             if (!mask_claim(refm, o, slot)) continue;         // (a reaction reading two changed species is listed twice)
-            if (mask_claim(advm, o, slot))                    // T_k += a_k dt with the OLD a_k, once
-              sT[li] = __dadd_rn(sT[li], __dmul_rn(sA[li], dprev));
+            // T_k += a_k dt with the OLD a_k, once: S1 has advanced exactly the owner's candidate and mu
+            double tk = t_old;
+            if (ob != k && k != mu_prev) {
+              tk = __dadd_rn(t_old, __dmul_rn(a_old, dprev));
+              sT[li] = tk;
+              atomicOr(&advm[o][slot >> 5], 1u << (slot & 31));
+            }
             sA[li] = a_new;
             if (filter_unsafe(a_new)) ctx.any_odd = 1;
             // A refreshed reaction invalidates its owner's proposal only if it IS that proposal;
             // otherwise its new waiting time joins the reduction as one more candidate.
-            if (mybest_k[o] == k || mybest_k[o] == -3 || k == mu_prev) {
+            if (ob == k || ob == -3 || k == mu_prev) {
               dirty[o] = 1;
             } else {
-              const double pk = sP[li], tk = sT[li];
               const double d = waiting_time(pk, tk, a_new);
               if (cand_less(d, k, extra)) { extra.dt = d; extra.k = k; }
               // The owner keeps its candidate while every other reaction of it stays clear of it (2^-13
