@@ -763,6 +763,38 @@ def test_ensemble_to_t_end_on_the_bundle_path(rt, pipeline, exchange):
     assert (g["stop"] == rt.RT_STOP_T_END).all() and (g["t"] == t_end).all()
 
 
+def test_kernels_agree_bit_for_bit_far_beyond_the_horizon(rt):
+    """1.5e5 firings of a cfg3-like network -- fifteen times the bit-exact horizon north_star sets
+    for GPU vs oracle.  Between host and device a one-ulp difference of a log grows tenfold every
+    ~1e4 firings until two events swap (reading G9; pinned on the oracle alone by
+    test_one_ulp_in_one_draw_bounds_the_bit_exact_horizon), so against the oracle only the first
+    5e4 firings are compared, with the drift of the event times inside that envelope.  But every
+    GPU path performs the SAME rounded operations in the same order, so all of them -- candidate-
+    first and pass-then-reduce kernel, cluster and L2 exchange, 1 to 16 CTAs, state on chip or in
+    global memory -- must agree with one another to the last bit over the whole run."""
+    net, x0, par = W.make_config("cfg3", scale=0.02)
+    nf = 150_000
+    o = _oracle().run(net, x0, par["seed"], 0, 50_000, math.inf, 50_000)
+    runs = []
+    for opts in ((), (("pipeline", 0),), (("exchange", 1),), (("bundle_ctas", 1),), (("bundle_ctas", 16),),
+                 (("state_mode", 1),), (("pipeline", 0), ("exchange", 1), ("bundle_ctas", 7))):
+        with rt.Model(net) as m:
+            for k, v in opts:
+                m.set_option(k, v)
+            runs.append(m.run(x0, par["seed"], 0, nf, math.inf, nf, want_state=True))
+    g = runs[0]
+    np.testing.assert_array_equal(g["trace_mu"][:50_000], o["trace_mu"])
+    rel = np.abs(g["trace_t"][:50_000] - o["trace_t"]) / o["trace_t"]
+    assert rel[:10_000].max() < RTOL_T and rel.max() < 1e-8
+    for h in runs[1:]:
+        np.testing.assert_array_equal(h["trace_mu"], g["trace_mu"])
+        np.testing.assert_array_equal(h["trace_t"], g["trace_t"])
+        np.testing.assert_array_equal(h["x"], g["x"])
+        np.testing.assert_array_equal(h["T"], g["T"])
+        np.testing.assert_array_equal(h["P"], g["P"])
+        np.testing.assert_array_equal(h["fire_count"], g["fire_count"])
+
+
 def test_options_are_validated_and_reported(rt):
     """Every tuning knob of rt.h: out-of-range values and unknown names are refused, accepted values
     show up in rt_get_info after a launch, and none of them changes a result."""
