@@ -42,6 +42,8 @@ extern "C" {
 #define RT_ERR_OVERFLOW     -5   /* a species count left [0, bound] during a run                 */
 #define RT_ERR_CUDA         -6   /* CUDA runtime error, no device, or an in-kernel barrier timeout */
 #define RT_ERR_OOM          -7   /* host or device allocation failed                             */
+#define RT_ERR_SCRATCH      -8   /* rt_run_dev_noalloc: rt_noalloc_prepare not called for this model, or
+                                    the run needs more than RT_NOALLOC_SCRATCH_BYTES of scratch       */
 
 /* ---- why a trajectory stopped (not errors) ------------------------------------------------- */
 #define RT_STOP_T_END        1   /* next firing would pass t_end: t = t_end, nothing fired        */
@@ -137,6 +139,40 @@ int rt_run_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t traje
                uint64_t max_firings, double t_end,
                int64_t *x_out_dev, rt_result *res_dev,
                int32_t *trace_mu_dev, double *trace_t_dev, uint64_t trace_cap, void *stream);
+
+/* ---- no-allocation entry point --------------------------------------------------------------
+ * For callers that may not call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it).  rt_run_dev keeps the per-trajectory scratch of the bundle kernels
+ * (Eq.15/24/26 state T, P, a [M], firing counts n [M], the versioned count words X [N] and the
+ * argmin exchange slots of PAPER.md:195-199, :211) in buffers it allocates on first use.
+ * rt_run_dev_noalloc is the same launch with that scratch in ONE file-scope array in device memory,
+ *   static __device__ __align__(256) unsigned char [RT_NOALLOC_SCRATCH_BYTES]   (4 MiB),
+ * which every GPU that loads the library holds until the process exits.  It calls no cudaMalloc,
+ * cudaFree or allocating library routine: it enqueues one memset of the exchange slots (they must
+ * start at zero; T, P, a, n, X are initialised by the kernel from x0_dev and the Philox stream) and
+ * one kernel on `stream`.  Need in bytes, each part rounded up to 256: 3*8*M_pad + 4*M_pad + 8*G*N +
+ * 512*S (M_pad = M rounded up to even; S = CTAs of the bundle, <= 160, two rounds of 256-byte
+ * exchange slots each; G = "x_replicas"), i.e. networks up to about M = 1.4e5: config 3 fits,
+ * config 4 does not.
+ * THE ARRAY IS SHARED: by every model on the device, every stream and every call.  It keeps the
+ * last call's contents, and two calls that overlap on the GPU (different streams, or the same
+ * model's rt_run_dev_noalloc twice without stream order) race on it: keep them in stream order.
+ *
+ * rt_noalloc_prepare: set-up, once per model after its options are set (it MAY allocate: the first
+ * call per device loads the kernels and takes the array's device address with
+ * cudaGetSymbolAddress).  *need_bytes (may be NULL) receives the scratch the current options need.
+ * Returns RT_ERR_SCRATCH if that exceeds RT_NOALLOC_SCRATCH_BYTES, RT_ERR_CUDA on a runtime error.
+ *
+ * rt_run_dev_noalloc: arguments, results and error reporting exactly as rt_run_dev (bit-identical
+ * outputs).  RT_ERR_SCRATCH if the model was not prepared or the launch shape the current options
+ * give needs more than RT_NOALLOC_SCRATCH_BYTES; nothing is enqueued then.  State streamed from
+ * global memory ("state_mode" = 1) runs without the persisting-L2 window of "l2_persist". */
+#define RT_NOALLOC_SCRATCH_BYTES (4u << 20)
+int rt_noalloc_prepare(rt_model *m, uint64_t *need_bytes);
+int rt_run_dev_noalloc(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t trajectory,
+                       uint64_t max_firings, double t_end,
+                       int64_t *x_out_dev, rt_result *res_dev,
+                       int32_t *trace_mu_dev, double *trace_t_dev, uint64_t trace_cap, void *stream);
 
 /* n_traj independent trajectories traj_first .. traj_first+n_traj-1 from the same x0 (the
  * paper's "bundles").  Row i of the outputs is exactly what

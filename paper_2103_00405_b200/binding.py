@@ -13,6 +13,8 @@ import numpy as np
 RT_OK = 0
 RT_ERR_NULL, RT_ERR_BAD_NETWORK, RT_ERR_BAD_ARG, RT_ERR_UNSUPPORTED = -1, -2, -3, -4
 RT_ERR_OVERFLOW, RT_ERR_CUDA, RT_ERR_OOM = -5, -6, -7
+RT_ERR_SCRATCH = -8
+RT_NOALLOC_SCRATCH_BYTES = 4 << 20
 RT_STOP_T_END, RT_STOP_MAX_FIRINGS, RT_STOP_ABSORBED = 1, 2, 3
 
 # rt_result: (f64 t, u64 firings, i32 stop, i32 status), 24 bytes
@@ -56,6 +58,8 @@ def lib():
     L.rt_run.argtypes = [vp, vp, u64, u64, u64, f64, vp, vp, vp, vp, vp, vp, vp, u64]
     L.rt_run_resume.argtypes = [vp, vp, f64, vp, vp, vp, u64, u64, u64, f64, vp, vp, vp, vp, vp, vp, vp, u64]
     L.rt_run_dev.argtypes = [vp, vp, u64, u64, u64, f64, vp, vp, vp, vp, u64, vp]
+    L.rt_run_dev_noalloc.argtypes = [vp, vp, u64, u64, u64, f64, vp, vp, vp, vp, u64, vp]
+    L.rt_noalloc_prepare.argtypes = [vp, C.POINTER(u64)]
     L.rt_ensemble.argtypes = [vp, vp, u64, u64, u64, u64, f64, vp, vp]
     L.rt_ensemble_dev.argtypes = [vp, vp, u64, u64, u64, u64, f64, vp, vp, vp]
     L.rt_sync.argtypes = [vp, vp]
@@ -68,7 +72,7 @@ def lib():
     L.rt_strerror.argtypes = [i32]
     L.rt_strerror.restype = C.c_char_p
     for name in ("rt_validate_network", "rt_create", "rt_run", "rt_run_resume", "rt_run_dev", "rt_ensemble", "rt_set_rate_schedule",
-                 "rt_set_rate_exponent",
+                 "rt_set_rate_exponent", "rt_run_dev_noalloc", "rt_noalloc_prepare",
                  "rt_ensemble_dev", "rt_sync", "rt_set_option", "rt_get_info"):
         getattr(L, name).restype = i32
     _lib = L
@@ -223,6 +227,22 @@ def rt_run_dev(handle, x0_dev, seed, trajectory, max_firings, t_end, x_out_dev, 
                             int(max_firings), float(t_end), _dev_ptr(x_out_dev), _dev_ptr(res_dev),
                             _dev_ptr(trace_mu_dev), _dev_ptr(trace_t_dev), int(trace_cap),
                             _stream_ptr())
+
+
+def rt_noalloc_prepare(handle):
+    """Set-up for rt_run_dev_noalloc (may allocate).  Returns (rc, scratch bytes the options need)."""
+    need = C.c_uint64(0)
+    rc = lib().rt_noalloc_prepare(C.c_void_p(handle), C.byref(need))
+    return rc, int(need.value)
+
+
+def rt_run_dev_noalloc(handle, x0_dev, seed, trajectory, max_firings, t_end, x_out_dev, res_dev,
+                       trace_mu_dev=None, trace_t_dev=None, trace_cap=0):
+    """rt_run_dev with its scratch in the library's static device array: no allocation in the call."""
+    return lib().rt_run_dev_noalloc(C.c_void_p(handle), _dev_ptr(x0_dev), int(seed), int(trajectory),
+                                    int(max_firings), float(t_end), _dev_ptr(x_out_dev), _dev_ptr(res_dev),
+                                    _dev_ptr(trace_mu_dev), _dev_ptr(trace_t_dev), int(trace_cap),
+                                    _stream_ptr())
 
 
 def rt_ensemble_dev(handle, x0_dev, seed, traj_first, n_traj, max_firings, t_end, x_out_dev, res_dev):

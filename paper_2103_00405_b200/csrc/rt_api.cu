@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -106,6 +107,7 @@ struct rt_model {
   int64_t kernel_launches = 0;
   int last_S = 0, last_B = 0, last_path = 0, last_state_smem = 0, last_block = 0;
   size_t n_big = 0;
+  unsigned char *noalloc_scratch = nullptr;   // device address of the static scratch array (rt_noalloc_prepare)
 };
 
 namespace {
@@ -942,8 +944,141 @@ const char *rt_strerror(int code) {
     case RT_ERR_OVERFLOW: return "species count left the supported range";
     case RT_ERR_CUDA: return "CUDA error or in-kernel barrier timeout";
     case RT_ERR_OOM: return "out of memory";
+    case RT_ERR_SCRATCH:
+      return "no-allocation entry point: rt_noalloc_prepare not called for this model, or the run "
+             "needs more than RT_NOALLOC_SCRATCH_BYTES of scratch";
     default: return "unknown error code";
   }
+}
+
+}  // extern "C"
+
+// ---- no-allocation entry point (include/rt.h: rt_noalloc_prepare / rt_run_dev_noalloc) ---------
+// The bundle kernels' scratch -- T, P, a, n, X and the exchange slots, which rt_run_dev keeps in
+// cudaMalloc'ed buffers (ensure_state) -- carved out of one file-scope array in device memory.
+// Every context that loads this module holds the array until it is destroyed.  In HOST code the
+// name below is only a handle for cudaGetSymbolAddress, never a device address.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[RT_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+unsigned char *g_noalloc_ptr[kNoallocMaxDevices] = {};   // the array's device address, per device
+
+struct ScratchLayout { size_t T, P, a, n, X, exch, exch_bytes, total; };
+
+ScratchLayout scratch_layout(const rt_model *m, const Plan &pl) {
+  auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
+  const size_t Mp = (size_t)m->net.M_pad, N = (size_t)m->net.N, B = (size_t)pl.B;
+  ScratchLayout L{};
+  size_t at = 0;
+  L.T = at; at += up(B * Mp * 8);
+  L.P = at; at += up(B * Mp * 8);
+  L.a = at; at += up(B * Mp * 8);
+  L.n = at; at += up(B * Mp * 4);
+  L.X = at; at += up(B * (size_t)pl.G * N * 8);
+  L.exch = at;
+  L.exch_bytes = B * 2 * (size_t)pl.S * rt::kSlotStride * 8;
+  at += up(L.exch_bytes);
+  L.total = at;
+  return L;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rt_noalloc_prepare(rt_model *m, uint64_t *need_bytes) {
+  if (!m) return RT_ERR_NULL;
+  if (m->device < 0 || m->device >= kNoallocMaxDevices) return RT_ERR_UNSUPPORTED;
+  CU_TRY(cudaSetDevice(m->device));
+  {
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[m->device]) {         // once per device, with that device current
+      unsigned char *ptr = nullptr;
+      CU_TRY(cudaGetSymbolAddress((void **)&ptr, g_noalloc_scratch));
+      if (!ptr) return RT_ERR_CUDA;
+      g_noalloc_ptr[m->device] = ptr;
+    }
+    m->noalloc_scratch = g_noalloc_ptr[m->device];
+  }
+  const Plan pl = plan_bundles(m, 1);        // (also asks the occupancy questions the plan caches)
+  const ScratchLayout L = scratch_layout(m, pl);
+  if (need_bytes) *need_bytes = (uint64_t)L.total;
+  if (L.total > (size_t)RT_NOALLOC_SCRATCH_BYTES) return RT_ERR_SCRATCH;
+  // load the kernel this plan launches now, outside the caller's no-allocation region
+  const int rate = m->sched_n > 0 ? 1 : m->rate_exp ? 2 : 0;
+  if (rate != 0 && (m->refresh_mode != 0 || m->opt_formulation != 0)) return RT_OK;   // (the run reports it)
+  const void *kern = bundle_kernel(pl.smem, m->refresh_mode != 0, rate, pl.cluster, pl.fast);
+  cudaFuncAttributes fa;
+  CU_TRY(cudaFuncGetAttributes(&fa, kern));
+  return RT_OK;
+}
+
+int rt_run_dev_noalloc(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t trajectory,
+                       uint64_t max_firings, double t_end, int64_t *x_out_dev, rt_result *res_dev,
+                       int32_t *trace_mu_dev, double *trace_t_dev, uint64_t trace_cap, void *stream) {
+  if (!m || !x0_dev || !res_dev) return RT_ERR_NULL;
+  int rc = check_limits(max_firings, t_end);
+  if (rc != RT_OK) return rc;
+  if (!m->noalloc_scratch) return RT_ERR_SCRATCH;
+  if (m->sched_n > 0 && (m->refresh_mode != 0 || m->opt_formulation != 0)) return RT_ERR_UNSUPPORTED;
+  if (m->rate_exp && (m->refresh_mode != 0 || m->opt_formulation != 0 || m->sched_n > 0)) return RT_ERR_UNSUPPORTED;
+  CU_TRY(cudaSetDevice(m->device));
+  cudaStream_t st = (cudaStream_t)stream;
+  const Plan pl = plan_bundles(m, 1);
+  const ScratchLayout L = scratch_layout(m, pl);
+  if (L.total > (size_t)RT_NOALLOC_SCRATCH_BYTES) return RT_ERR_SCRATCH;
+  unsigned char *base = m->noalloc_scratch;
+  // the array keeps the last call's contents: the exchange slots must start at zero (their tags
+  // would otherwise match a new round); everything else is written by the kernel before it is read
+  CU_TRY(cudaMemsetAsync(base + L.exch, 0, L.exch_bytes, st));
+  rt::BundleParams p{};
+  p.net = m->net;
+  p.T = (double *)(base + L.T); p.P = (double *)(base + L.P); p.a = (double *)(base + L.a);
+  p.n = (uint32_t *)(base + L.n); p.X = (u64 *)(base + L.X);
+  p.exch = (u64 *)(base + L.exch);
+  p.S = pl.S; p.B = pl.B; p.G = pl.G; p.pairs_per_cta = pl.pairs_per_cta; p.cnt_pad = pl.cnt_pad;
+  p.x0 = (const long long *)x0_dev; p.seed = seed; p.traj_first = trajectory; p.n_traj = 1;
+  p.max_firings = max_firings; p.t_end = t_end;
+  p.x_out = (long long *)x_out_dev; p.res = res_dev;
+  p.trace_mu = trace_mu_dev; p.trace_t = trace_t_dev;
+  p.trace_cap = (trace_mu_dev || trace_t_dev) ? trace_cap : 0;
+  p.refresh_mode = m->refresh_mode;
+  p.prefetch = m->opt_prefetch;
+  p.formulation = m->opt_formulation;
+  p.rate_lambda = (const double *)m->d_lambda.p;
+  p.sched_n = m->sched_n;
+  p.sched_t = (const double *)m->d_sched_t.p;
+  p.sched_f = (const double *)m->d_sched_f.p;
+  p.sched_mask = m->sched_has_mask ? (const unsigned char *)m->d_sched_mask.p : nullptr;
+  p.err = (int *)m->d_err.p;                 // (16 bytes owned by the model since rt_create)
+  void *args[] = {&p};
+  const int rate = m->sched_n > 0 ? 1 : m->rate_exp ? 2 : 0;
+  const void *kern = bundle_kernel(pl.smem, m->refresh_mode != 0, rate, pl.cluster, pl.fast);
+  const size_t dyn = pl.smem ? smem_state_bytes(pl.pairs_per_cta, pl.fast) : 0;
+  if (dyn) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+  const int block = pl.fast ? kBlockFast : pl.smem ? kBlockSmem : kBlockGlobal;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(pl.S * pl.B); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = dyn; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  if (pl.cluster) {
+    if (pl.S > 8) CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = pl.S; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  } else {
+    at[0].id = cudaLaunchAttributeCooperative;
+    at[0].val.cooperative = 1;
+  }
+  cfg.attrs = at; cfg.numAttrs = 1;
+  CU_TRY(cudaLaunchKernelExC(&cfg, kern, args));
+  m->last_block = block;
+  m->kernel_launches += 1;
+  m->last_S = pl.S; m->last_B = pl.B; m->last_path = 2; m->last_state_smem = pl.smem ? 1 : 0;
+  m->last_cluster = pl.cluster ? 1 : 0;
+  m->last_fast = pl.fast ? 1 : 0;
+  return RT_OK;
 }
 
 }  // extern "C"
