@@ -85,3 +85,62 @@ REFERENCE_OPTIONS = [("pipeline", 0), ("bundle_ctas", 1), ("state_mode", 1), ("p
                      ("refresh_mode", 1)]
 
 INF = math.inf
+
+
+# ---- cases for the other entry points and modes (tests/test_gpu_fuzz.py, second test) ---------
+SIMPLE_OPTIONS = [("pipeline", 0), ("bundle_ctas", 1), ("state_mode", 1), ("prefetch", 0)]
+MODES = ["ensemble", "ensemble", "resume", "residual", "schedule", "exponential"]
+
+
+def make_mode_case(seed):
+    """A dict: mode, net, x0, options, firings, trajectory, plus what the mode needs.  Relative
+    quantities (fractions of the run's duration) are resolved by the test once it knows that
+    duration; nothing here depends on the method."""
+    r = np.random.default_rng(7919 * seed + 3)
+    mode = MODES[int(r.integers(0, len(MODES)))]
+    c = dict(mode=mode, seed=seed)
+    if mode == "ensemble":
+        which = int(r.integers(0, 3))          # 0: <= 4 reactions (register kernel), 1: <= 64, 2: bundle kernel
+        if which == 0:
+            net, x0 = W.random_mass_action(int(r.integers(1, 5)), int(r.integers(1, 5)), seed=seed)
+            x0 = r.integers(0, 300, size=len(x0)).astype(np.int64)
+        elif which == 1:
+            net, x0 = W.random_mass_action(int(r.integers(1, 33)), int(r.integers(1, 65)), seed=seed)
+            if r.random() < 0.4:
+                x0 = r.integers(0, 40, size=len(x0)).astype(np.int64)
+        else:
+            net, x0, _, _, _ = make_case(seed, max_reactions=20_000)
+        opts = []
+        if which == 1 and r.random() < 0.3:
+            opts.append(("ensemble_path", 2))
+        if which == 0 and r.random() < 0.3:
+            opts.append(("tiny_kernel", 0))
+        if which == 2:
+            if r.random() < 0.5:
+                opts.append(("pipeline", int(r.integers(0, 2))))
+            if r.random() < 0.5:
+                opts.append(("exchange", int(r.integers(0, 2))))
+            if r.random() < 0.5:
+                opts.append(("bundle_ctas", int(r.choice([0, 1, 2, 3, 7, 13, 16]))))
+        c.update(net=dict(net), x0=np.ascontiguousarray(x0, dtype=np.int64), options=opts,
+                 n_traj=int(r.choice([1, 2, 31, 33, 64, 200])) if which < 2 else int(r.integers(1, 24)),
+                 firings=int(10 ** r.uniform(1.5, 3.0)), traj_first=int(r.integers(0, 5000)),
+                 t_end_fraction=float(r.uniform(0.3, 1.2)) if r.random() < 0.4 else None,
+                 drop_firing_limit=bool(r.random() < 0.5))
+        return c
+    net, x0, opts, firings, traj = make_case(seed, max_reactions=40_000)
+    opts = [o for o in opts if o[0] != "refresh_mode"]
+    c.update(net=net, x0=x0, options=opts, firings=min(firings, 1500), trajectory=traj)
+    M = int(net["n_reactions"])
+    if mode in ("resume", "residual"):
+        c["split"] = float(r.uniform(0.1, 0.9))
+    elif mode == "schedule":
+        nb = int(r.integers(1, 8))
+        c["break_fractions"] = np.sort(r.uniform(0.0, 1.1, size=nb))
+        if r.random() < 0.2:
+            c["break_fractions"][0] = 0.0
+        c["factor"] = r.choice([0.0, 0.5, 1.0, 2.0, 3.7], size=nb)
+        c["mask"] = None if r.random() < 0.5 else (r.random(M) < 0.5).astype(np.uint8)
+    else:
+        c["lambda_times_duration"] = r.choice([0.0, 1.0, -1.0, 0.3, -2.5], size=M)
+    return c

@@ -142,3 +142,119 @@ def test_a_known_sensitive_case_is_checked_through_its_resyncs(rt):
     one-ulp redraw is amplified past the 1e-12 bar, so that the check above has to follow the GPU
     run through resyncs instead of passing on the first comparison."""
     assert _fuzz_one(rt, 136) >= 1
+
+
+# ---- the other entry points and modes ----------------------------------------------------------
+def _bitwise_common(g, h, what):
+    for k in ("firings", "stop", "x", "trace_mu", "fire_count"):
+        if k in g and g[k] is not None and k in h and h[k] is not None:
+            np.testing.assert_array_equal(np.asarray(g[k]), np.asarray(h[k]), err_msg=f"{what}: {k}")
+    for k in ("t", "trace_t"):
+        if k in g and g[k] is not None and k in h and h[k] is not None:
+            np.testing.assert_array_equal(_bits(g[k]), _bits(h[k]), err_msg=f"{what}: {k}")
+
+
+def _at_the_bar(g, o):
+    ok = (np.array_equal(np.asarray(g["firings"]), np.asarray(o["firings"]))
+          and np.array_equal(np.asarray(g["stop"]), np.asarray(o["stop"]))
+          and np.array_equal(g["x"], o["x"])
+          and np.allclose(np.asarray(g["t"]), np.asarray(o["t"]), rtol=RTOL_T, atol=0))
+    if ok and g.get("trace_mu") is not None:
+        n = len(o["trace_mu"])
+        ok = (len(g["trace_mu"]) == n and np.array_equal(g["trace_mu"], o["trace_mu"])
+              and np.allclose(g["trace_t"], o["trace_t"], rtol=RTOL_T, atol=0)
+              and np.array_equal(g["fire_count"], o["fire_count"]))
+    return ok
+
+
+def _mode_one(rt, seed):
+    """Returns True if the case also meets the oracle at the bar (it always must match the simplest
+    GPU variant bit for bit), None if the generated case is degenerate (nothing happens in it)."""
+    import oracle
+    from helpers.fuzz_cases import make_mode_case, SIMPLE_OPTIONS
+    c = make_mode_case(seed)
+    net, x0, opts, firings, mode = c["net"], c["x0"], c["options"], c["firings"], c["mode"]
+    what = f"seed {seed} {mode} {opts}"
+    if mode == "ensemble":
+        t_end = INF
+        if c["t_end_fraction"] is not None:
+            t1 = oracle.run(net, x0, seed, 0, firings, INF, 0, check=False)["t"]
+            t_end = t1 * c["t_end_fraction"] if t1 > 0 else 1.0
+            if c["drop_firing_limit"]:
+                firings = 0
+        try:
+            o = oracle.ensemble(net, x0, seed, c["traj_first"], c["n_traj"], firings, t_end, n_threads=4)
+        except RuntimeError:
+            return None                     # (a count overflow: covered by its own parity test)
+        with rt.Model(net) as m:
+            for k, v in opts:
+                m.set_option(k, v)
+            g = m.ensemble(x0, seed, c["traj_first"], c["n_traj"], firings, t_end, check=False)
+        with rt.Model(net) as m:
+            for k, v in (("ensemble_path", 2), ("pipeline", 0), ("bundle_ctas", 1)):
+                m.set_option(k, v)
+            h = m.ensemble(x0, seed, c["traj_first"], c["n_traj"], firings, t_end, check=False)
+        _bitwise_common(g, h, what)
+        return _at_the_bar(g, o)
+    traj = c["trajectory"]
+    plain = oracle.run(net, x0, seed, traj, firings, INF, 0, check=False)
+    if plain["code"] != 0 or plain["t"] <= 0.0:
+        return None
+    duration = plain["t"]
+
+    def configure(m, options):
+        for k, v in options:
+            m.set_option(k, v)
+        if mode == "residual":
+            m.set_option("formulation", 1)
+        elif mode == "schedule":
+            m.set_rate_schedule(tb, c["factor"], c["mask"])
+        elif mode == "exponential":
+            m.set_rate_exponent(lam)
+
+    if mode == "schedule":
+        tb = c["break_fractions"] * duration
+        if len(np.unique(tb)) != len(tb):
+            return None
+        o = oracle.run_sched(net, x0, seed, traj, firings, INF, firings, t_break=tb, factor=c["factor"],
+                             mask=c["mask"])
+    elif mode == "exponential":
+        lam = c["lambda_times_duration"] / duration
+        o = oracle.run_rate_exp(net, x0, lam, seed, traj, firings, INF, firings)
+    elif mode == "residual":
+        o = oracle.run_residual(net, x0, seed, traj, firings, INF, firings)
+    else:
+        o = oracle.run(net, x0, seed, traj, firings, INF, firings, check=False)
+    with rt.Model(net) as m:
+        configure(m, opts)
+        if mode in ("resume", "residual"):
+            n1 = max(1, min(firings - 1, int(firings * c["split"])))
+            a = m.run(x0, seed, traj, n1, INF, n1, want_state=True, check=False)
+            b = m.run_resume(a["x"], a["t"], a["T"], a["P"], a["fire_count"], seed, traj, firings - n1, INF,
+                             firings - n1, want_state=True, check=False)
+            g = dict(x=b["x"], t=b["t"], firings=a["firings"] + b["firings"], stop=b["stop"],
+                     trace_mu=np.concatenate([a["trace_mu"], b["trace_mu"]]),
+                     trace_t=np.concatenate([a["trace_t"], b["trace_t"]]), fire_count=b["fire_count"])
+        else:
+            g = m.run(x0, seed, traj, firings, INF, firings, want_state=True, check=False)
+    with rt.Model(net) as m:
+        configure(m, SIMPLE_OPTIONS)
+        h = m.run(x0, seed, traj, firings, INF, firings, want_state=True, check=False)     # (in one piece)
+    _bitwise_common(g, h, what)
+    return _at_the_bar(g, o)
+
+
+@pytest.mark.parametrize("chunk", range(8))
+def test_random_cases_of_the_other_modes(rt, chunk):
+    """Ensembles (register, shared-memory and bundle kernels; firing and time limits), checkpoint /
+    resume in both formulations, rate schedules and exponential rates on random networks and
+    options: each case bit for bit against the simplest variant of the library run in one piece,
+    and against the oracle at the bar.  The one-ulp differences between host and device log
+    (module docstring) are not followed through resyncs here; during development 2 % of 10 000
+    such cases left the bar because of them (each one bit-identical to the simplest variant),
+    none for any other reason; of the 240 cases here one does.  A chunk of 30 may miss the bar in at
+    most two cases."""
+    results = [_mode_one(rt, seed) for seed in range(1 + chunk * 30, 1 + (chunk + 1) * 30)]
+    ran = [x for x in results if x is not None]
+    assert len(ran) >= 20
+    assert sum(1 for x in ran if not x) <= 2, results
