@@ -274,6 +274,10 @@ Plan plan_bundles_for(rt_model *m, u64 n_traj, bool fast) {
     // longer pass of fewer, fuller CTAs.
     const int sc = std::min(rt::kMaxClusterCtas, s_thin);
     if (may_cluster && sc >= 2 && sc >= s_fit && max_active_clusters(m, sc) >= 1) S = sc;
+    // Through L2 every lane of the exchange warp polls ceil(S / 32) slots: with the pass hidden behind
+    // the exchange (candidate-first kernel) 128 CTAs with 4 slots per lane beat 148 with 5 (cfg4: 3.16
+    // against 3.23 us per firing; 119..128 alike, 129 already slower), if the state still fits.
+    else if (fast && m->opt_state_mode != 1 && S == sms && S % 32 != 0 && S / 32 * 32 >= s_fit) S = S / 32 * 32;
   } else {
     S = (int)std::max<u64>(1, (u64)sms / n_traj);       // many: as many bundles as fit ...
     if (m->opt_state_mode != 1 && S < s_fit && s_fit <= sms) S = s_fit;   // ... with on-chip state

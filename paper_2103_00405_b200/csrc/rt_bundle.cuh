@@ -36,8 +36,14 @@ namespace rt {
 constexpr int kListCap = 256;       // refreshed reactions a CTA stages per round
 constexpr int kWalkerWarps = 1;
 constexpr int kMaxBundleCtas = 160; // CTAs that may share one trajectory (5 exchange slots per lane)
-constexpr int kSlotStride = 32;     // u64 words between exchange slots: 256 B, so the 148 slots that every
-                                    // CTA polls spread over as many L2 slices instead of queueing on a few
+#ifndef RT_SLOT_STRIDE
+#define RT_SLOT_STRIDE 128
+#endif
+// u64 words between exchange slots: 1 KiB, so that the slots every CTA polls spread over as many L2
+// slices instead of queueing on a few.  Measured (tests/helpers/exchange_floor.cu with this stride,
+// 148 CTAs): 16 B..128 B apart 2.3-3.2 us per round (posters share lines), 256 B 1.23 us, 1 KiB
+// 1.02 us, 4 KiB 1.06 us; in the kernel cfg4 3.26 -> 3.23 us, cfg5b +1.5 %.
+constexpr int kSlotStride = RT_SLOT_STRIDE;
 
 struct BundleParams {
   NetDev net;

@@ -6,7 +6,7 @@
 // NOTHING else is done between rounds -- i.e. the latency one firing pays for its argmin exchange
 // (the bundle-level reduction) however fast the pass is:
 //   l2      S CTAs post to slots in global memory (L2), each CTA polls all S slots
-//           (st.relaxed.gpu / ld.relaxed.gpu, 256 B slot stride, double-buffered by round parity;
+//           (st.relaxed.gpu / ld.relaxed.gpu, slot stride SLOT_STRIDE words, double-buffered by round parity;
 //           a lane's loads are all in flight together, as in rt_bundle.cuh)
 //   l2push  each CTA writes its word into a private row of every reader (S x S slots), so that a
 //           polled line has ONE reader and is written by one CTA per slot
@@ -31,7 +31,10 @@
 #include <cooperative_groups.h>
 
 typedef unsigned long long u64;
-constexpr int kSlotStride = 32;   // u64 words: 256 B
+#ifndef SLOT_STRIDE
+#define SLOT_STRIDE 128
+#endif
+constexpr int kSlotStride = SLOT_STRIDE;   // u64 words between slots: 1 KiB as in rt_bundle.cuh (-DSLOT_STRIDE=32: 256 B)
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { \
   printf("CUDA error %s at %s:%d\n", cudaGetErrorString(e_), __FILE__, __LINE__); exit(1); } } while (0)
@@ -329,9 +332,11 @@ int main() {
 
   printf("mode,ctas,cluster,n_clusters,us_per_round\n");
   for (int push = 0; push < 2; ++push)
-    for (int S : {1, 2, 4, 8, 16, 37, 74, 148}) {
+    for (int S : {1, 2, 4, 8, 16, 37, 74, 96, 128, 148}) {
       cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3(S); cfg.blockDim = dim3(32); cfg.dynamicSmemBytes = 0;
+      const void *fn = push ? (const void *)k_l2<true> : (const void *)k_l2<false>;
+      CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+      cfg.gridDim = dim3(S); cfg.blockDim = dim3(32); cfg.dynamicSmemBytes = dyn;   // one CTA per SM
       cudaLaunchAttribute at[1];
       at[0].id = cudaLaunchAttributeCooperative; at[0].val.cooperative = 1;
       cfg.attrs = at; cfg.numAttrs = 1;
