@@ -511,8 +511,10 @@ struct Spec {
 // slots in L2.  Doubles as the per-firing bundle barrier.  On return every lane holds the
 // bundle-wide winner in `c` (c.k == -2: timeout) and the runner-up in `c2`.
 // `between` runs after this CTA has posted and before it waits (work hidden behind the exchange).
+// DEFER2: `c2` comes back as each lane's contribution to the runner-up; the caller reduces it
+// (warp_lexmin) after it has published the winner, off the critical path of the firing.
 struct NoWork { __device__ __forceinline__ void operator()() const {} };
-template <bool CLUSTER, typename Between = NoWork>
+template <bool CLUSTER, typename Between = NoWork, bool DEFER2 = false>
 __device__ __forceinline__ void exchange_partials(const BundleParams &p, u64 (*cl_slot)[kMaxClusterCtas][2],
                                                   u64 *cl_bar, u64 *exch, int r, uint32_t gen, int lane,
                                                   Cand &c, Cand &c2, Between between = Between()) {
@@ -540,7 +542,7 @@ __device__ __forceinline__ void exchange_partials(const BundleParams &p, u64 (*c
     }
     c = warp_lexmin(s);
     if (s.k == c.k) { s.dt = __longlong_as_double(0x7ff0000000000000ll); s.k = 0x7fffffff; }
-    c2 = warp_lexmin(s);                        // runner-up: best of everything but the winner
+    c2 = DEFER2 ? s : warp_lexmin(s);           // runner-up: best of everything but the winner
     if (__any_sync(0xffffffffu, timed_out)) c.k = -2;
   } else if (p.S > 1) {
     const uint32_t tag = gen + 1u;
@@ -578,7 +580,8 @@ __device__ __forceinline__ void exchange_partials(const BundleParams &p, u64 (*c
     const Cand mine_best = c;
     c = warp_lexmin(c);
     // runner-up = best of everything but the winner: the likeliest winner of the next firing
-    c2 = warp_lexmin((mine_best.k == c.k) ? c2 : mine_best);
+    c2 = (mine_best.k == c.k) ? c2 : mine_best;
+    if (!DEFER2) c2 = warp_lexmin(c2);
     if (timed_out) c.k = -2;
   }
 }

@@ -72,7 +72,8 @@ template <int BLOCK>
 struct FastCtx {
   Cand warp_part[(BLOCK - 32 * kFastHelperWarps) / 32];
   Cand win;
-  int second_k;
+  u64 second;             // L2 exchange: runner-up tagged with its generation, (gen << 32) | k
+  int second_k;           // cluster: runner-up of the exchange (published with the winner)
   int abort_local, list_n, list_buf, more, any_odd;
   alignas(16) u64 cl_slot[2][kMaxClusterCtas][2];
   alignas(8) u64 cl_bar[2];
@@ -194,7 +195,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
   uint32_t gen = 0;
   if (tid == 0) {
     ctx.abort_local = 0; ctx.list_n = 0; ctx.list_buf = 0; ctx.more = 0; ctx.any_odd = 0;
-    ctx.second_k = 0x7fffffff;
+    ctx.second = ~0ull; ctx.second_k = 0x7fffffff;
   }
   if (CLUSTER && tid == 0) {
     mbar_init(smem_addr(&ctx.cl_bar[0]), 1u);
@@ -247,6 +248,8 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
     int cur = 0;                         // staged-list buffer this firing publishes
     // walker warp: what it has prepared for the likely next winner
     int k2 = 0x7fffffff;                 //   runner-up of the last exchange
+    bool want2 = false;                  //   ... still to be fetched from ctx.second (tag tag2)
+    uint32_t tag2 = 0u;
     int pw_k = -1, pw_n = 0;             //   pre-walked reaction: its entries in [k0, k1) are in pw_d / pw_c
     int4 pw_ent = make_int4(-1, 0, 0, 0);//   its stoich row (lanes 0..3)
     bool sp_valid = false, sp_bad = false;  // speculative refreshes of pw_k in out_*[1 - cur], computed
@@ -559,10 +562,21 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         c = warp_lexmin(c);
         const Cand mine = c;
         Cand c2;
-        exchange_partials<CLUSTER>(p, ctx.cl_slot, ctx.cl_bar, exch, r, gen, lane, c, c2);
-        if (lane == 0) { ctx.win = c; ctx.second_k = (c2.dt < INF) ? c2.k : 0x7fffffff; }
+        // Through L2 the runner-up is reduced after the winner is out: only the walker wants it, and
+        // later (cfg4 3.16 -> 3.12 us, cfg5b +3 %).  In a cluster the walker is the busiest warp of
+        // the firing and would wait for it: there it is published together with the winner.
+        constexpr bool kDefer2 = !CLUSTER;
+        exchange_partials<CLUSTER, NoWork, kDefer2>(p, ctx.cl_slot, ctx.cl_bar, exch, r, gen, lane, c, c2);
+        if (lane == 0) ctx.win = c;
+        if (!kDefer2 && lane == 0) ctx.second_k = (c2.dt < INF) ? c2.k : 0x7fffffff;
         named_arrive<BLOCK>(kBarWin);
         win = c;
+        if (kDefer2) {
+          c2 = warp_lexmin(c2);
+          if (lane == 0)
+            *reinterpret_cast<volatile u64 *>(&ctx.second) =
+                ((u64)gen << 32) | (u64)(uint32_t)((c2.dt < INF) ? c2.k : 0x7fffffff);
+        }
         // every CTA will need the candidate's stoich row and the dependency entries of its species,
         // all DRAM-cold (each reaction fires rarely): pull them into L2, once per candidate
         if (mine.k != pf_k && mine.k < M && (p.prefetch & 1)) {
@@ -583,6 +597,12 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         if (is_walker) {
           // ===== walker: prepare the likely next winner k2 while the others reduce and exchange
           // (1) its dependency entries in [k0, k1) (network data): row -> ranges -> entries
+          if (want2) {                   // (written by the exchange warp right after the last winner)
+            u64 v;
+            do { v = *reinterpret_cast<volatile u64 *>(&ctx.second); } while ((uint32_t)(v >> 32) != tag2);
+            k2 = (int)(uint32_t)v;
+            want2 = false;
+          }
           if ((p.prefetch & 4) && k2 != pw_k && k2 < M && k1 > k0) {
             pw_k = -1;
             int4 ent = make_int4(-1, 0, 0, 0);
@@ -649,7 +669,10 @@ __global__ void __launch_bounds__(BLOCK, 1) rt_fast_kernel(const BundleParams p)
         }
         named_sync<BLOCK>(kBarWin);
         win = ctx.win;
-        if (is_walker) k2 = ctx.second_k;
+        if (is_walker) {
+          if (CLUSTER) k2 = ctx.second_k;
+          else { want2 = true; tag2 = gen; }
+        }
       }
       gen += 1u;
       cur ^= 1;
