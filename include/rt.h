@@ -152,7 +152,7 @@ int rt_run_dev(rt_model *m, const int64_t *x0_dev, uint64_t seed, uint64_t traje
  * start at zero; T, P, a, n, X are initialised by the kernel from x0_dev and the Philox stream) and
  * one kernel on `stream`.  Need in bytes, each part rounded up to 256: 3*8*M_pad + 4*M_pad + 8*G*N +
  * 2048*S (M_pad = M rounded up to even; S = CTAs of the bundle, <= 160, two rounds of 1 KiB
- * exchange slots each; G = "x_replicas"), i.e. networks up to about M = 1.4e5: config 3 fits,
+ * exchange slots each; G = "x_replicas"), i.e. networks up to about M = 1.3e5: config 3 fits,
  * config 4 does not.
  * THE ARRAY IS SHARED: by every model on the device, every stream and every call.  It keeps the
  * last call's contents, and two calls that overlap on the GPU (different streams, or the same
